@@ -1,0 +1,143 @@
+/* fdtd_b200.h — C ABI of the B200-native 3-D acoustic FDTD + CPML time step.
+ *
+ * The operation is one time step of the staggered-grid, radius-4 (8th-order) pressure-velocity update of
+ * PAPER.md section 3.1 with the CPML memory-variable recursion of section 3.2 in the
+ * outer absorbing layer, parameters of Table 2.  P:NN = line NN of the paper text; Rn = a
+ * reading listed in DESIGN.md where the paper is silent or ambiguous.
+ *
+ * Conventions
+ *   - Total grid N_a = n_interior[a] + cpml[2a] + cpml[2a+1]; x fastest: idx = i + Nx (j + Ny k).
+ *   - p lives on nodes (i,j,k); vx on (i+1/2,j,k); vy on (i,j+1/2,k); vz on (i,j,k+1/2) (R1, R3).
+ *   - All fields are fp32.  Every pointer argument says HOST or DEVICE.
+ *   - Every entry point except fdtd_create / fdtd_workspace_bytes / fdtd_last_error returns 0 on success
+ *     and a negative FDTD_E* code on error; on error the context is left unchanged.  CUDA errors are
+ *     captured and returned (FDTD_ECUDA), never abort().  No exception crosses this boundary.
+ *   - Nothing here has a CPU fallback: without a CUDA device every compute call fails with FDTD_ECUDA.
+ *   - Work is enqueued on params.stream; calls are asynchronous unless the comment says "synchronises".
+ */
+#ifndef FDTD_B200_H
+#define FDTD_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fdtd_ctx fdtd_ctx; /* opaque */
+
+enum {
+  FDTD_OK = 0,
+  FDTD_EINVAL = -1,     /* bad size / parameter (dt <= 0, grid smaller than the layers, source out of range ...) */
+  FDTD_EWORKSPACE = -2, /* workspace NULL, misaligned (256 B) or smaller than fdtd_workspace_bytes() */
+  FDTD_ECUDA = -3,      /* a CUDA runtime / driver call failed; fdtd_last_error() has the text */
+  FDTD_EUNSUPPORTED = -4 /* valid per the paper but not built (e.g. heterogeneous density, R6 / NEXT-3) */
+};
+
+enum { FDTD_P = 0, FDTD_VX = 1, FDTD_VY = 2, FDTD_VZ = 3 };                 /* field selectors */
+enum { FDTD_PSI_VX = 0, FDTD_PSI_VY = 1, FDTD_PSI_VZ = 2, FDTD_PSI_PX = 3, FDTD_PSI_PY = 4, FDTD_PSI_PZ = 5 };
+enum { FDTD_WALL = 0, FDTD_PERIODIC = 1 };
+enum {
+  FDTD_KERNEL_AUTO = 0, /* TMA-staged, z-streaming tile kernels (the product path)                        */
+  FDTD_KERNEL_REF = 1   /* one thread per point, global loads only; also the only path for FDTD_PERIODIC   */
+};
+
+/* Problem statement and Table 2 as one plain-data block. */
+typedef struct {
+  int32_t n_interior[3];  /* interior cells x, y, z                                                        */
+  int32_t cpml[6];        /* CPML thickness per global face x-,x+,y-,y+,z-,z+ in cells; 0 = plain wall (R13) */
+  double dx, dt;          /* cubic cell size; time step chosen by the caller (Courant * dx / c_max, R15)    */
+  int32_t cpml_order;     /* q: grading order (P:50 uses 3; BASELINE configs use 2)                         */
+  int32_t boundary;       /* FDTD_WALL: reads outside the grid return 0 (R4); FDTD_PERIODIC: wrap (tests)   */
+  double cpml_R0;         /* target reflection R of sigma_max                                 */
+  double cpml_kappa_max;  /* kappa_max                                                        */
+  double cpml_alpha_max;  /* alpha_max                                                        */
+  double cpml_c_ref;      /* wave speed absorbed into sigma_max = -(q+1) c_ref ln(R0) / (2 L dx) (R7)        */
+  int32_t decomp[3];      /* in-HBM subdomain grid; {1,1,1} (or zeros) = monolithic.  decomp[0] must be 1:   */
+                          /* pencil-yz keeps x local                                                  */
+  int32_t ghost;          /* ghost depth g in cells on every internal interface                 */
+  int32_t substeps_per_exchange; /* m sub-updates (v or p) between halo exchanges; needs g >= 4 m (R20)      */
+  int32_t kernel;         /* FDTD_KERNEL_AUTO / FDTD_KERNEL_REF                                              */
+  int32_t device;         /* CUDA device ordinal                                                             */
+  void* stream;           /* cudaStream_t the work is enqueued on (0 = legacy default stream)                */
+  void* workspace;        /* DEVICE memory, 256-byte aligned, owned by the caller, must outlive the context  */
+  uint64_t workspace_bytes;
+} fdtd_params;
+
+/* Bytes of device workspace fdtd_create needs for these parameters (fields p, vx, vy, vz, the per-node
+ * K dt/dx array, slab-local psi arrays, CPML tables, source tables, halo buffers).  0 on invalid parameters.
+ * Reads only the size fields; no CUDA call. */
+uint64_t fdtd_workspace_bytes(const fdtd_params* params);
+
+/* Builds a context: lays the arrays out in params->workspace, zero-fills fields and psi (BASELINE config 1:
+ * "fields initialised to zero"), computes the CPML tables b = exp[-(sigma/kappa + alpha) dt],
+ * a = sigma (b-1) / [kappa (sigma + kappa alpha)] in double on the host and uploads them as fp32,
+ * sets the homogeneous medium c = rho = 1, step counter 0.  Returns NULL on error (see fdtd_last_error). */
+fdtd_ctx* fdtd_create(const fdtd_params* params);
+
+/* Medium (R6): c and rho are HOST arrays of the total grid (Nz*Ny*Nx fp32, x fastest) or NULL for 1.0
+ * everywhere.  The library forms K dt/dx = rho c^2 dt/dx per node and dt/(rho dx) (double arithmetic, rounded
+ * once to fp32) and copies them to the device before returning (synchronises the stream).  A non-uniform rho
+ * returns FDTD_EUNSUPPORTED. */
+int fdtd_set_model(fdtd_ctx* ctx, const float* c_host, const float* rho_host);
+
+/* Point sources injected into p (P:193 gives the Ricker shape; R14): after the pressure sub-update of step n,
+ * p[ijk_s] += wavelets[s*len + n]; steps n >= len inject nothing.  ijk: HOST, 3*n total-grid indices;
+ * wavelets: HOST, n*len fp32.  Copied before return (synchronises the stream).  n = 0 clears the sources. */
+int fdtd_set_sources(fdtd_ctx* ctx, int32_t n, const int32_t* ijk_host, const float* wavelets_host, int32_t len);
+
+/* Advances n time steps: for each step the velocity sub-update v_a -= (dt/rho)[(1/kappa_a) D+_a p + psi_va],
+ * psi_va <- b psi_va + a D+_a p, then the pressure sub-update
+ * p -= K dt sum_a [(1/kappa_a) D-_a v_a + psi_pa] (the z term per R2), then the source.  In subdomain
+ * mode a halo exchange (pack / copy / unpack) runs every substeps_per_exchange sub-updates.
+ * Asynchronous on params.stream; no host synchronisation. */
+int fdtd_step(fdtd_ctx* ctx, int32_t n);
+
+/* Copies one field (FDTD_P..FDTD_VZ) of the total grid, unpadded, to dst_host (Nz*Ny*Nx fp32).  In subdomain
+ * mode the owned cells of every subdomain are gathered.  Synchronises the stream. */
+int fdtd_get_field(fdtd_ctx* ctx, int32_t which, float* dst_host);
+
+/* Sub-box [lo, lo+size) of one field to dst_host (size[2]*size[1]*size[0] fp32, x fastest).  Synchronises. */
+int fdtd_get_field_box(fdtd_ctx* ctx, int32_t which, const int32_t lo[3], const int32_t size[3], float* dst_host);
+
+/* Overwrites one field from a HOST array of the total grid (initial conditions for tests).  In subdomain mode
+ * ghost cells are filled consistently.  Synchronises. */
+int fdtd_set_field(fdtd_ctx* ctx, int32_t which, const float* src_host);
+
+/* Fills one field on the device with the counter-based generator scale * u(seed + (which << 56), global linear
+ * index), u = top 24 bits of splitmix64 mapped to [-1, 1) — synthetic initial states at any grid size
+ * (DESIGN.md "Input recipe").  Asynchronous. */
+int fdtd_fill_hash(fdtd_ctx* ctx, int32_t which, uint64_t seed, double scale);
+
+/* One CPML memory variable (FDTD_PSI_*) expanded from its slab-local storage to the full total grid (zeros
+ * outside the slabs) into dst_host — debugging / parity of the recursion.  Synchronises. */
+int fdtd_get_psi(fdtd_ctx* ctx, int32_t which, float* dst_host);
+
+/* max |f| over the box [lo, lo+size) of one field, reduced on the device; result to *out_host.  Synchronises. */
+int fdtd_field_absmax(fdtd_ctx* ctx, int32_t which, const int32_t lo[3], const int32_t size[3], float* out_host);
+
+/* The CPML tables of one axis (0..2) and one staggering (half = 1: v family at i+1/2; 0: p family at nodes), as
+ * uploaded: a, b, 1/kappa, each N_axis fp32 into HOST arrays (R8).  Outside the layer a = 0, b = 1,
+ * 1/kappa = 1. */
+int fdtd_cpml_table(fdtd_ctx* ctx, int32_t axis, int32_t half, float* a_host, float* b_host, float* ik_host);
+
+/* The four staggered difference weights c_1..c_4 as the kernels use them (fp32; BASELINE: bit-exact). */
+int fdtd_coeffs(float out_host[4]);
+
+/* Number of kernel launches (the library's own kernels) enqueued since the context was created. */
+int64_t fdtd_launch_count(const fdtd_ctx* ctx);
+
+/* Total grid extents. */
+int fdtd_dims(const fdtd_ctx* ctx, int32_t out[3]);
+
+/* Releases the context (not the workspace).  Synchronises the stream first. */
+int fdtd_destroy(fdtd_ctx* ctx);
+
+/* Text of the last error on the calling thread ("" if none). */
+const char* fdtd_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FDTD_B200_H */

@@ -1,0 +1,747 @@
+// Host side of the C ABI declared in include/fdtd_b200.h: workspace layout, CPML coefficient setup,
+// TMA descriptors, launch orchestration of one time step, halo exchange of the in-HBM subdomain mode
+// (P:76-82).  No CPU fallback: every compute entry point needs a CUDA device.
+#include "../../include/fdtd_b200.h"
+#include "fdtd_kernels.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+
+using namespace fdtd;
+
+namespace {
+
+thread_local std::string g_err;
+void set_err(const std::string& s) { g_err = s; }
+
+#define CK(call)                                                                                   \
+  do {                                                                                             \
+    cudaError_t e_ = (call);                                                                       \
+    if (e_ != cudaSuccess) {                                                                       \
+      set_err(std::string(#call) + ": " + cudaGetErrorString(e_));                                 \
+      return FDTD_ECUDA;                                                                           \
+    }                                                                                              \
+  } while (0)
+
+inline uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
+inline int round_up(int v, int a) { return (v + a - 1) / a * a; }
+
+// ---- CPML tables (readings R7-R9) -------------------------------------------------------------
+struct AxisTable { std::vector<float> a, b, ik; };
+
+AxisTable make_axis_table(int N, int L0, int L1, bool half, const fdtd_params& P) {
+  AxisTable t;
+  const int len = round_up(N, 4) + 4;
+  t.a.assign(len, 0.0f); t.b.assign(len, 1.0f); t.ik.assign(len, 1.0f);
+  const double q = (double)P.cpml_order;
+  for (int i = 0; i < N; ++i) {
+    const double pos = i + (half ? 0.5 : 0.0);
+    double rho = 0.0; int L = 0;
+    if (L0 > 0 && L0 - pos > 0.0) { rho = (L0 - pos) / L0; L = L0; }                              // low face
+    else if (L1 > 0 && pos - (N - 1 - L1) > 0.0) { rho = (pos - (N - 1 - L1)) / L1; L = L1; }     // high face
+    if (L == 0) continue;
+    const double smax = -(q + 1.0) * P.cpml_c_ref * std::log(P.cpml_R0) / (2.0 * L * P.dx);
+    const double rq = std::pow(rho, q);
+    const double sig = smax * rq;
+    const double kap = 1.0 + (P.cpml_kappa_max - 1.0) * rq;
+    const double alp = P.cpml_alpha_max * std::fmax(0.0, 1.0 - rho);
+    const double bb = std::exp(-(sig / kap + alp) * P.dt);
+    const double den = kap * (sig + kap * alp);
+    t.a[i] = (float)(den == 0.0 ? 0.0 : sig * (bb - 1.0) / den);
+    t.b[i] = (float)bb;
+    t.ik[i] = (float)(1.0 / kap);
+  }
+  return t;
+}
+
+// ---- geometry ------------------------------------------------------------------------------------------
+struct Geometry {
+  int gn[3];                 // global total grid
+  int nd[3];                 // subdomain grid
+  int ghost, msub;
+  // global CPML storage slabs per axis: low [0, gs0), high [gh, gn) (x rounded to multiples of 4)
+  int gs0[3], gh[3];
+  bool valid = false;
+  std::string why;
+};
+
+Geometry make_geometry(const fdtd_params& P) {
+  Geometry G;
+  auto bad = [&](const char* w) { G.valid = false; G.why = w; return G; };
+  for (int a = 0; a < 3; ++a) {
+    if (P.n_interior[a] <= 0) return bad("n_interior must be positive");
+    if (P.cpml[2 * a] < 0 || P.cpml[2 * a + 1] < 0) return bad("cpml thickness must be >= 0");
+    long long n = (long long)P.n_interior[a] + P.cpml[2 * a] + P.cpml[2 * a + 1];
+    if (n > 100000) return bad("axis too long");
+    G.gn[a] = (int)n;
+    G.nd[a] = P.decomp[a] <= 0 ? 1 : P.decomp[a];
+  }
+  if (!(P.dx > 0.0) || !(P.dt > 0.0)) return bad("dx and dt must be positive");
+  if (P.boundary != FDTD_WALL && P.boundary != FDTD_PERIODIC) return bad("unknown boundary");
+  if (P.boundary == FDTD_PERIODIC)
+    for (int f = 0; f < 6; ++f) if (P.cpml[f]) return bad("PERIODIC excludes CPML");
+  for (int f = 0; f < 6; ++f)
+    if (P.cpml[f] > 0 && (!(P.cpml_R0 > 0.0) || P.cpml_order < 1 || !(P.cpml_kappa_max >= 1.0) || P.cpml_alpha_max < 0.0 || !(P.cpml_c_ref > 0.0)))
+      return bad("bad CPML parameters");
+  if (G.nd[0] != 1) return bad("decomp[0] must be 1 (pencil-yz keeps x local)");
+  const bool sub = G.nd[1] * G.nd[2] > 1;
+  G.ghost = sub ? P.ghost : 0;
+  G.msub = sub ? P.substeps_per_exchange : 0;
+  if (sub) {
+    if (P.boundary == FDTD_PERIODIC) return bad("subdomain mode needs WALL boundaries");
+    if (G.msub < 1 || G.ghost < 4 * G.msub) return bad("ghost must be >= 4 * substeps_per_exchange");
+    for (int a = 1; a < 3; ++a) {
+      if (G.gn[a] % G.nd[a]) return bad("total grid not divisible by decomp");
+      if (G.gn[a] / G.nd[a] < G.ghost) return bad("ghost deeper than a subdomain");
+    }
+  }
+  for (int a = 0; a < 3; ++a) {
+    const int L0 = P.cpml[2 * a], L1 = P.cpml[2 * a + 1];
+    int s0 = L0, h = L1 > 0 ? G.gn[a] - 1 - L1 : G.gn[a];
+    if (a == 0) { s0 = std::min(round_up(s0, 4), round_up(G.gn[a], 4)); h = h / 4 * 4; }
+    if (h < 0) h = 0;
+    if (L0 > 0 && L1 > 0 && s0 > h) return bad("grid smaller than its CPML layers");
+    G.gs0[a] = s0; G.gh[a] = h;
+  }
+  G.valid = true;
+  return G;
+}
+
+// One domain on the host: its view plus what the launches need.
+struct Domain {
+  DomainView v;
+  int own_lo[3], own_hi[3];    // owned cells in local indices
+  int cy, cz;                  // position in the subdomain grid
+  CUtensorMap tm_p, tm_vy;
+  long long* src_offset = nullptr;   // device, per source
+};
+
+struct Layout {
+  uint64_t total = 0;
+  struct Dom {
+    int n[3], o[3], pitch;
+    int ls[3][2], ln[3][2];
+    uint64_t f[4], kc, psi[2][3][2], src_off;
+  };
+  std::vector<Dom> doms;
+  uint64_t tab[2][3][3];
+  int tablen[3];
+  uint64_t step, wav, absmax, halo;
+  uint64_t halo_bytes;
+};
+
+constexpr int MAX_SRC = 64;
+constexpr int MAX_WAV_FLOATS = 1 << 22;
+
+Layout make_layout(const fdtd_params& P, const Geometry& G) {
+  Layout L;
+  uint64_t off = 0;
+  auto take = [&](uint64_t bytes) { uint64_t o = off; off = align_up(off + bytes, 256); return o; };
+  for (int cz = 0; cz < G.nd[2]; ++cz)
+    for (int cy = 0; cy < G.nd[1]; ++cy) {
+      Layout::Dom d{};
+      const int c[3] = {0, cy, cz};
+      for (int a = 0; a < 3; ++a) {
+        const int own = G.gn[a] / G.nd[a];
+        const int glo = c[a] > 0 ? G.ghost : 0, ghi = c[a] < G.nd[a] - 1 ? G.ghost : 0;
+        d.n[a] = own + glo + ghi;
+        d.o[a] = c[a] * own - glo;
+        // local parts of the global storage slabs
+        const int lo_end = std::min(G.gs0[a], d.o[a] + d.n[a]);       // global end of the low slab inside this domain
+        d.ls[a][0] = 0; d.ln[a][0] = (P.cpml[2 * a] > 0 && d.o[a] < G.gs0[a]) ? std::max(0, lo_end - d.o[a]) : 0;
+        const int hi_beg = std::max(G.gh[a], d.o[a]);
+        d.ls[a][1] = hi_beg - d.o[a];
+        d.ln[a][1] = (P.cpml[2 * a + 1] > 0 && d.o[a] + d.n[a] > G.gh[a]) ? std::max(0, d.o[a] + d.n[a] - hi_beg) : 0;
+        if (d.ln[a][1] == 0) d.ls[a][1] = 0;
+      }
+      if (d.ln[0][0] > 0) d.ln[0][0] = round_up(d.ln[0][0], 4);
+      if (d.ln[0][1] > 0) d.ln[0][1] = round_up(d.n[0] - d.ls[0][1], 4);
+      d.pitch = round_up(d.n[0], 8);
+      const uint64_t vol = (uint64_t)d.pitch * d.n[1] * d.n[2] * 4;
+      for (int f = 0; f < 4; ++f) d.f[f] = take(vol);
+      d.kc = take(vol);
+      for (int fam = 0; fam < 2; ++fam)
+        for (int s = 0; s < 2; ++s) {
+          d.psi[fam][0][s] = take((uint64_t)d.ln[0][s] * d.n[1] * d.n[2] * 4 + 16);
+          d.psi[fam][1][s] = take((uint64_t)d.pitch * d.ln[1][s] * d.n[2] * 4 + 16);
+          d.psi[fam][2][s] = take((uint64_t)d.pitch * d.n[1] * d.ln[2][s] * 4 + 16);
+        }
+      d.src_off = take(MAX_SRC * sizeof(long long));
+      L.doms.push_back(d);
+    }
+  for (int a = 0; a < 3; ++a) {
+    L.tablen[a] = round_up(G.gn[a], 4) + 4;
+    for (int fam = 0; fam < 2; ++fam)
+      for (int t = 0; t < 3; ++t) L.tab[fam][a][t] = take((uint64_t)L.tablen[a] * 4);
+  }
+  L.step = take(64);
+  L.absmax = take(64);
+  L.wav = take((uint64_t)MAX_WAV_FLOATS * 4);
+  // halo staging: one contiguous send buffer per exchange: the largest face set of 4 fields + psi
+  L.halo_bytes = 0;
+  if (G.nd[1] * G.nd[2] > 1) {
+    uint64_t mx = 0;
+    for (auto& d : L.doms) {
+      const uint64_t fy = (uint64_t)d.n[0] * G.ghost * d.n[2], fz = (uint64_t)d.n[0] * d.n[1] * G.ghost;
+      mx = std::max(mx, std::max(fy, fz));
+    }
+    L.halo_bytes = mx * 4 * 16;   // 4 fields + up to 12 psi pieces, generous
+  }
+  L.halo = take(L.halo_bytes + 16);
+  L.total = off;
+  return L;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+}  // namespace
+
+struct fdtd_ctx {
+  fdtd_params P;
+  Geometry G;
+  Layout L;
+  char* ws;
+  cudaStream_t stream;
+  std::vector<Domain> doms;
+  AxisTable tabs[2][3];
+  bool use_ref;
+  int nsrc = 0, wlen = 0;
+  long long* d_step;
+  float* d_wav;
+  int64_t launches = 0;
+  int64_t substeps_done = 0;    // sub-updates since the last halo exchange (subdomain mode)
+  int zchunk_v = 0, zchunk_p = 0;
+  int nchunk_v = 1, nchunk_p = 1;
+};
+
+namespace {
+
+int make_tmap(EncodeTiledFn enc, CUtensorMap* m, float* base, const DomainView& v, int bw, int bh) {
+  cuuint64_t dims[3] = {(cuuint64_t)v.nx, (cuuint64_t)v.ny, (cuuint64_t)v.nz};
+  cuuint64_t strides[2] = {(cuuint64_t)v.pitch * 4, (cuuint64_t)v.plane * 4};
+  cuuint32_t box[3] = {(cuuint32_t)bw, (cuuint32_t)bh, 1};
+  cuuint32_t estr[3] = {1, 1, 1};
+  CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                   CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { set_err("cuTensorMapEncodeTiled failed with CUresult " + std::to_string((int)r)); return FDTD_ECUDA; }
+  return FDTD_OK;
+}
+
+int pick_chunks(fdtd_ctx* c, const void* kernel, int smem, int nz, int tiles_xy, int* zchunk, int* nchunk) {
+  int per_sm = 0, dev = c->P.device, sms = 148;
+  CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, NT, smem));
+  CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  const long long cap = (long long)std::max(per_sm, 1) * sms;
+  int n;
+  if (const char* e = getenv("FDTD_ZCHUNK")) {
+    n = std::max(1, (nz + atoi(e) - 1) / std::max(1, atoi(e)));
+  } else if (tiles_xy >= cap) {
+    n = std::max(1, (nz + 127) / 128);                 // many waves: short chunks keep the tail small
+  } else {
+    n = (int)std::max(1LL, cap / tiles_xy);            // one wave: as many equal chunks as fit
+    n = std::min(n, std::max(1, nz / 8));
+  }
+  *zchunk = (nz + n - 1) / n;
+  *nchunk = (nz + *zchunk - 1) / *zchunk;
+  return FDTD_OK;
+}
+
+int launch_substep(fdtd_ctx* c, Domain& d, int which /*0 = v, 1 = p*/) {
+  const DomainView& v = d.v;
+  if (c->use_ref) {
+    dim3 b(64, 4, 1), g((v.nx + 63) / 64, (v.ny + 3) / 4, v.nz);
+    if (which == 0) update_v_ref<<<g, b, 0, c->stream>>>(v);
+    else update_p_ref<<<g, b, 0, c->stream>>>(v);
+  } else {
+    dim3 g((v.nx + TX - 1) / TX, (v.ny + TY - 1) / TY, which == 0 ? c->nchunk_v : c->nchunk_p);
+    if (which == 0) update_v_tiled<<<g, NT, V_SMEM_BYTES, c->stream>>>(d.tm_p, v, c->zchunk_v);
+    else update_p_tiled<<<g, NT, P_SMEM_BYTES, c->stream>>>(d.tm_vy, v, c->zchunk_p);
+  }
+  c->launches++;
+  CK(cudaGetLastError());
+  return FDTD_OK;
+}
+
+int launch_inject(fdtd_ctx* c) {
+  if (c->nsrc == 0) return FDTD_OK;   // the step counter only matters to the wavelet index
+  for (size_t k = 0; k < c->doms.size(); ++k) {
+    SourceView S{c->nsrc, c->wlen, c->doms[k].src_offset, c->doms[k].v.f[0], c->d_wav, c->d_step};
+    inject_sources<<<1, 64, 0, c->stream>>>(S, k + 1 == c->doms.size());
+    c->launches++;
+  }
+  CK(cudaGetLastError());
+  return FDTD_OK;
+}
+
+// ---- halo exchange between in-HBM subdomains (pack -> copy -> unpack; here one fused copy kernel per
+// phase because source and destination share one address space) --------------------------------------
+struct CopyJob {
+  const float* src; float* dst;
+  long long sp, sr, dp, dr;   // plane / row strides (floats) of source and destination
+  int w, h, d;                // box size: w floats per row (multiple of 4), h rows, d planes
+};
+constexpr int MAX_JOBS = 24;
+struct CopyBatch { CopyJob job[MAX_JOBS]; int n; };
+
+__global__ void __launch_bounds__(256) halo_copy_kernel(const __grid_constant__ CopyBatch B) {
+  const CopyJob& J = B.job[blockIdx.y];
+  const int w4 = J.w >> 2;
+  const long long n = (long long)w4 * J.h * J.d;
+  for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
+    const int x = (int)(t % w4);
+    const long long r = t / w4;
+    const int y = (int)(r % J.h), z = (int)(r / J.h);
+    const float4 val = *reinterpret_cast<const float4*>(J.src + z * J.sp + y * J.sr + 4 * x);
+    *reinterpret_cast<float4*>(J.dst + z * J.dp + y * J.dr + 4 * x) = val;
+  }
+}
+
+int run_batch(fdtd_ctx* c, const CopyBatch& B) {
+  if (B.n == 0) return FDTD_OK;
+  long long mx = 0;
+  for (int i = 0; i < B.n; ++i) mx = std::max(mx, (long long)(B.job[i].w / 4) * B.job[i].h * B.job[i].d);
+  const int bx = (int)std::min<long long>(std::max<long long>((mx + 255) / 256, 1), 148 * 4);
+  halo_copy_kernel<<<dim3(bx, B.n), 256, 0, c->stream>>>(B);
+  c->launches++;
+  CK(cudaGetLastError());
+  return FDTD_OK;
+}
+
+// Adds the jobs that refresh `dst`'s ghost cells on its low/high side of `axis` (1 = y, 2 = z) from the owner.
+// Phase y copies owned rows over the owned z range only; phase z then copies whole planes (all local rows of the
+// receiving domain, ghost rows included), which carries the corners (R21).
+void add_face_jobs(fdtd_ctx* c, std::vector<CopyJob>& jobs, Domain& dst, Domain& src, int axis, int side) {
+  const DomainView &dv = dst.v, &sv = src.v;
+  const int g = c->G.ghost;
+  // destination ghost range along `axis` in dst-local indices, and the same cells in src-local indices
+  const int dlo = side == 0 ? 0 : dst.own_hi[axis];
+  const int glo_global = (axis == 1 ? dv.oy : dv.oz) + dlo;
+  const int slo = glo_global - (axis == 1 ? sv.oy : sv.oz);
+  auto push = [&](const float* sb, float* db, long long sp, long long sr, long long dp, long long dr, int w, int h, int d,
+                  long long soff, long long doff) {
+    if (w <= 0 || h <= 0 || d <= 0) return;
+    jobs.push_back(CopyJob{sb + soff, db + doff, sp, sr, dp, dr, w, h, d});
+  };
+  // z range / y range of the box in dst-local and src-local coordinates
+  int dy0, dy1, dz0, dz1;
+  if (axis == 1) { dy0 = dlo; dy1 = dlo + g; dz0 = dst.own_lo[2]; dz1 = dst.own_hi[2]; }
+  else { dy0 = 0; dy1 = dv.ny; dz0 = dlo; dz1 = dlo + g; }
+  const int sy0 = dy0 + dv.oy - sv.oy, sz0 = dz0 + dv.oz - sv.oz;
+  (void)slo;
+  const int w = dv.pitch;   // whole rows: x is never decomposed, both pitches are equal
+  for (int f = 0; f < 4; ++f)
+    push(sv.f[f], dv.f[f], sv.plane, sv.pitch, dv.plane, dv.pitch, w, dy1 - dy0, dz1 - dz0,
+         (long long)sz0 * sv.plane + (long long)sy0 * sv.pitch, (long long)dz0 * dv.plane + (long long)dy0 * dv.pitch);
+  // psi pieces that live in the ghost box (R21): x slabs (all j,k), y slabs (rows in slab), z slabs (planes in slab)
+  for (int fam = 0; fam < 2; ++fam) {
+    for (int s = 0; s < 2; ++s) {
+      if (dv.ln[0][s] > 0 && sv.ln[0][s] == dv.ln[0][s]) {
+        const int wx = dv.ln[0][s];
+        push(sv.psi[fam][0][s], dv.psi[fam][0][s], (long long)sv.ny * wx, wx, (long long)dv.ny * wx, wx, wx, dy1 - dy0, dz1 - dz0,
+             ((long long)sz0 * sv.ny + sy0) * wx, ((long long)dz0 * dv.ny + dy0) * wx);
+      }
+      // y-slab rows inside the box
+      if (dv.ln[1][s] > 0) {
+        const int a0 = std::max(dy0, dv.ls[1][s]), a1 = std::min(dy1, dv.ls[1][s] + dv.ln[1][s]);
+        if (a1 > a0 && sv.ln[1][s] > 0) {
+          const int sa0 = a0 + dv.oy - sv.oy;
+          if (sa0 >= sv.ls[1][s] && sa0 + (a1 - a0) <= sv.ls[1][s] + sv.ln[1][s])
+            push(sv.psi[fam][1][s], dv.psi[fam][1][s], (long long)sv.ln[1][s] * sv.pitch, sv.pitch, (long long)dv.ln[1][s] * dv.pitch,
+                 dv.pitch, w, a1 - a0, dz1 - dz0, ((long long)sz0 * sv.ln[1][s] + (sa0 - sv.ls[1][s])) * sv.pitch,
+                 ((long long)dz0 * dv.ln[1][s] + (a0 - dv.ls[1][s])) * dv.pitch);
+        }
+      }
+      // z-slab planes inside the box
+      if (dv.ln[2][s] > 0) {
+        const int a0 = std::max(dz0, dv.ls[2][s]), a1 = std::min(dz1, dv.ls[2][s] + dv.ln[2][s]);
+        if (a1 > a0 && sv.ln[2][s] > 0) {
+          const int sa0 = a0 + dv.oz - sv.oz;
+          if (sa0 >= sv.ls[2][s] && sa0 + (a1 - a0) <= sv.ls[2][s] + sv.ln[2][s])
+            push(sv.psi[fam][2][s], dv.psi[fam][2][s], (long long)sv.ny * sv.pitch, sv.pitch, (long long)dv.ny * dv.pitch, dv.pitch, w,
+                 dy1 - dy0, a1 - a0, ((long long)(sa0 - sv.ls[2][s]) * sv.ny + sy0) * sv.pitch,
+                 ((long long)(a0 - dv.ls[2][s]) * dv.ny + dy0) * dv.pitch);
+        }
+      }
+    }
+  }
+}
+
+int exchange_halos(fdtd_ctx* c) {
+  if (c->doms.size() <= 1) return FDTD_OK;
+  const int ny = c->G.nd[1], nz = c->G.nd[2];
+  for (int axis = 1; axis <= 2; ++axis) {
+    std::vector<CopyJob> jobs;
+    for (auto& d : c->doms) {
+      const int pos = axis == 1 ? d.cy : d.cz, cnt = axis == 1 ? ny : nz;
+      for (int side = 0; side < 2; ++side) {
+        const int npos = pos + (side == 0 ? -1 : 1);
+        if (npos < 0 || npos >= cnt) continue;
+        Domain& src = c->doms[axis == 1 ? (size_t)d.cz * ny + npos : (size_t)npos * ny + d.cy];
+        add_face_jobs(c, jobs, d, src, axis, side);
+      }
+    }
+    for (size_t b = 0; b < jobs.size(); b += MAX_JOBS) {
+      CopyBatch B{};
+      B.n = (int)std::min<size_t>(MAX_JOBS, jobs.size() - b);
+      for (int i = 0; i < B.n; ++i) B.job[i] = jobs[b + i];
+      int r = run_batch(c, B);
+      if (r) return r;
+    }
+  }
+  return FDTD_OK;
+}
+
+int do_substep(fdtd_ctx* c, int which) {
+  if (c->doms.size() > 1 && c->substeps_done % c->G.msub == 0) {
+    int r = exchange_halos(c);
+    if (r) return r;
+  }
+  for (auto& d : c->doms) {
+    int r = launch_substep(c, d, which);
+    if (r) return r;
+  }
+  c->substeps_done++;
+  return FDTD_OK;
+}
+
+// gather / scatter between a packed host total-grid array and the domains
+int copy_field(fdtd_ctx* c, float* const* dom_base, float* host, bool to_host, bool owned_only) {
+  const int gnx = c->G.gn[0], gny = c->G.gn[1];
+  for (auto& d : c->doms) {
+    const DomainView& v = d.v;
+    const int jl = owned_only ? d.own_lo[1] : 0, jh = owned_only ? d.own_hi[1] : v.ny;
+    const int kl = owned_only ? d.own_lo[2] : 0, kh = owned_only ? d.own_hi[2] : v.nz;
+    float* base = dom_base[&d - &c->doms[0]];
+    for (int k = kl; k < kh; ++k) {
+      float* dev = base + (long long)k * v.plane + (long long)jl * v.pitch;
+      float* h = host + ((long long)(k + v.oz) * gny + (jl + v.oy)) * gnx;
+      if (to_host) CK(cudaMemcpy2DAsync(h, (size_t)gnx * 4, dev, (size_t)v.pitch * 4, (size_t)v.nx * 4, jh - jl, cudaMemcpyDeviceToHost, c->stream));
+      else CK(cudaMemcpy2DAsync(dev, (size_t)v.pitch * 4, h, (size_t)gnx * 4, (size_t)v.nx * 4, jh - jl, cudaMemcpyHostToDevice, c->stream));
+    }
+  }
+  CK(cudaStreamSynchronize(c->stream));
+  return FDTD_OK;
+}
+
+}  // namespace
+
+// =========================================================================================== C ABI
+extern "C" {
+
+const char* fdtd_last_error(void) { return g_err.c_str(); }
+
+int fdtd_coeffs(float out[4]) {
+  if (!out) return FDTD_EINVAL;
+  out[0] = FDTD_C1; out[1] = FDTD_C2; out[2] = FDTD_C3; out[3] = FDTD_C4;
+  return FDTD_OK;
+}
+
+uint64_t fdtd_workspace_bytes(const fdtd_params* P) {
+  if (!P) return 0;
+  Geometry G = make_geometry(*P);
+  if (!G.valid) { set_err(G.why); return 0; }
+  return make_layout(*P, G).total;
+}
+
+fdtd_ctx* fdtd_create(const fdtd_params* P) {
+  if (!P) { set_err("params is NULL"); return nullptr; }
+  Geometry G = make_geometry(*P);
+  if (!G.valid) { set_err(G.why); return nullptr; }
+  Layout L = make_layout(*P, G);
+  if (!P->workspace || ((uintptr_t)P->workspace & 255) || P->workspace_bytes < L.total) {
+    set_err("workspace NULL, misaligned or too small (need " + std::to_string(L.total) + " bytes)");
+    return nullptr;
+  }
+  auto fail = [&](fdtd_ctx* c, cudaError_t e, const char* what) -> fdtd_ctx* {
+    set_err(std::string(what) + ": " + cudaGetErrorString(e));
+    delete c;
+    return nullptr;
+  };
+  fdtd_ctx* c = new fdtd_ctx();
+  c->P = *P; c->G = G; c->L = L;
+  c->ws = (char*)P->workspace;
+  c->stream = (cudaStream_t)P->stream;
+  c->use_ref = P->kernel == FDTD_KERNEL_REF || P->boundary == FDTD_PERIODIC;
+  cudaError_t e;
+  if ((e = cudaSetDevice(P->device)) != cudaSuccess) return fail(c, e, "cudaSetDevice");
+  if ((e = cudaMemsetAsync(c->ws, 0, L.total, c->stream)) != cudaSuccess) return fail(c, e, "cudaMemsetAsync(workspace)");
+
+  // CPML tables: double on the host, rounded once to fp32 (a6)
+  for (int a = 0; a < 3; ++a)
+    for (int fam = 0; fam < 2; ++fam) {
+      c->tabs[fam][a] = make_axis_table(G.gn[a], P->cpml[2 * a], P->cpml[2 * a + 1], fam == 0, *P);
+      const AxisTable& t = c->tabs[fam][a];
+      const float* src[3] = {t.a.data(), t.b.data(), t.ik.data()};
+      for (int k = 0; k < 3; ++k)
+        if ((e = cudaMemcpyAsync(c->ws + L.tab[fam][a][k], src[k], (size_t)L.tablen[a] * 4, cudaMemcpyHostToDevice, c->stream)) != cudaSuccess)
+          return fail(c, e, "cudaMemcpyAsync(tables)");
+    }
+  if ((e = cudaStreamSynchronize(c->stream)) != cudaSuccess) return fail(c, e, "cudaStreamSynchronize");
+
+  c->d_step = (long long*)(c->ws + L.step);
+  c->d_wav = (float*)(c->ws + L.wav);
+
+  EncodeTiledFn enc = nullptr;
+  if (!c->use_ref) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    if ((e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr)) != cudaSuccess || !fn)
+      return fail(c, e, "cudaGetDriverEntryPoint(cuTensorMapEncodeTiled)");
+    enc = (EncodeTiledFn)fn;
+  }
+
+  size_t di = 0;
+  for (int cz = 0; cz < G.nd[2]; ++cz)
+    for (int cy = 0; cy < G.nd[1]; ++cy, ++di) {
+      const Layout::Dom& ld = L.doms[di];
+      Domain d{};
+      DomainView& v = d.v;
+      v.nx = ld.n[0]; v.ny = ld.n[1]; v.nz = ld.n[2];
+      v.pitch = ld.pitch; v.plane = (long long)ld.pitch * ld.n[1];
+      v.ox = ld.o[0]; v.oy = ld.o[1]; v.oz = ld.o[2];
+      for (int a = 0; a < 3; ++a) v.gn[a] = G.gn[a];
+      v.periodic = P->boundary == FDTD_PERIODIC;
+      for (int f = 0; f < 4; ++f) v.f[f] = (float*)(c->ws + ld.f[f]);
+      v.kc = nullptr;
+      v.kc0 = (float)(1.0 * 1.0 * 1.0 * P->dt / P->dx);
+      v.b0 = (float)(P->dt / (1.0 * P->dx));
+      for (int a = 0; a < 3; ++a)
+        for (int s = 0; s < 2; ++s) {
+          v.ls[a][s] = ld.ls[a][s]; v.ln[a][s] = ld.ln[a][s];
+          for (int fam = 0; fam < 2; ++fam) v.psi[fam][a][s] = (float*)(c->ws + ld.psi[fam][a][s]);
+        }
+      for (int fam = 0; fam < 2; ++fam)
+        for (int a = 0; a < 3; ++a)
+          for (int k = 0; k < 3; ++k) v.tab[fam][a][k] = (const float*)(c->ws + L.tab[fam][a][k]);
+      d.cy = cy; d.cz = cz;
+      const int cc[3] = {0, cy, cz};
+      for (int a = 0; a < 3; ++a) {
+        d.own_lo[a] = cc[a] > 0 ? G.ghost : 0;
+        d.own_hi[a] = d.own_lo[a] + G.gn[a] / G.nd[a];
+      }
+      d.src_offset = (long long*)(c->ws + ld.src_off);
+      if (!c->use_ref) {
+        if (make_tmap(enc, &d.tm_p, v.f[0], v, VW, VH) || make_tmap(enc, &d.tm_vy, v.f[2], v, PW, PH)) { delete c; return nullptr; }
+      }
+      c->doms.push_back(d);
+    }
+
+  if (!c->use_ref) {
+    if ((e = cudaFuncSetAttribute(update_v_tiled, cudaFuncAttributeMaxDynamicSharedMemorySize, V_SMEM_BYTES)) != cudaSuccess)
+      return fail(c, e, "cudaFuncSetAttribute(update_v_tiled)");
+    if ((e = cudaFuncSetAttribute(update_p_tiled, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM_BYTES)) != cudaSuccess)
+      return fail(c, e, "cudaFuncSetAttribute(update_p_tiled)");
+    const DomainView& v0 = c->doms[0].v;
+    const int tiles = ((v0.nx + TX - 1) / TX) * ((v0.ny + TY - 1) / TY);
+    if (pick_chunks(c, (const void*)update_v_tiled, V_SMEM_BYTES, v0.nz, tiles, &c->zchunk_v, &c->nchunk_v) ||
+        pick_chunks(c, (const void*)update_p_tiled, P_SMEM_BYTES, v0.nz, tiles, &c->zchunk_p, &c->nchunk_p)) { delete c; return nullptr; }
+  }
+  return c;
+}
+
+int fdtd_dims(const fdtd_ctx* c, int32_t out[3]) {
+  if (!c || !out) return FDTD_EINVAL;
+  for (int a = 0; a < 3; ++a) out[a] = c->G.gn[a];
+  return FDTD_OK;
+}
+
+int64_t fdtd_launch_count(const fdtd_ctx* c) { return c ? c->launches : -1; }
+
+int fdtd_set_model(fdtd_ctx* c, const float* c_host, const float* rho_host) {
+  if (!c) return FDTD_EINVAL;
+  const size_t n = (size_t)c->G.gn[0] * c->G.gn[1] * c->G.gn[2];
+  double rho = 1.0;
+  if (rho_host) {
+    rho = rho_host[0];
+    for (size_t q = 1; q < n; ++q)
+      if (rho_host[q] != rho_host[0]) { set_err("heterogeneous density is not built (NEXT-3)"); return FDTD_EUNSUPPORTED; }
+    if (!(rho > 0.0)) { set_err("rho must be positive"); return FDTD_EINVAL; }
+  }
+  const float b0 = (float)(c->P.dt / (rho * c->P.dx));
+  if (!c_host) {
+    for (auto& d : c->doms) { d.v.kc = nullptr; d.v.kc0 = (float)(rho * 1.0 * 1.0 * c->P.dt / c->P.dx); d.v.b0 = b0; }
+    return FDTD_OK;
+  }
+  std::vector<float> kc(n);
+  for (size_t q = 0; q < n; ++q) {
+    const double cc = c_host[q];
+    if (!(cc > 0.0)) { set_err("c must be positive"); return FDTD_EINVAL; }
+    kc[q] = (float)(rho * cc * cc * c->P.dt / c->P.dx);     // K dt/dx = rho c^2 dt/dx (R6), rounded once
+  }
+  std::vector<float*> bases;
+  for (size_t k = 0; k < c->doms.size(); ++k) bases.push_back((float*)(c->ws + c->L.doms[k].kc));
+  int r = copy_field(c, bases.data(), kc.data(), false, false);
+  if (r) return r;
+  for (size_t k = 0; k < c->doms.size(); ++k) { c->doms[k].v.kc = bases[k]; c->doms[k].v.b0 = b0; }
+  return FDTD_OK;
+}
+
+int fdtd_set_sources(fdtd_ctx* c, int32_t n, const int32_t* ijk, const float* wav, int32_t len) {
+  if (!c || n < 0 || n > MAX_SRC) { set_err("bad source count"); return FDTD_EINVAL; }
+  if (n == 0) { c->nsrc = 0; c->wlen = 0; return FDTD_OK; }
+  if (!ijk || !wav || len <= 0 || (long long)n * len > MAX_WAV_FLOATS) { set_err("bad source table"); return FDTD_EINVAL; }
+  for (int s = 0; s < n; ++s)
+    for (int a = 0; a < 3; ++a)
+      if (ijk[3 * s + a] < 0 || ijk[3 * s + a] >= c->G.gn[a]) { set_err("source outside the grid"); return FDTD_EINVAL; }
+  for (auto& d : c->doms) {
+    std::vector<long long> off(n, -1);
+    for (int s = 0; s < n; ++s) {
+      const int li = ijk[3 * s] - d.v.ox, lj = ijk[3 * s + 1] - d.v.oy, lk = ijk[3 * s + 2] - d.v.oz;
+      if (li >= 0 && li < d.v.nx && lj >= 0 && lj < d.v.ny && lk >= 0 && lk < d.v.nz)
+        off[s] = (long long)lk * d.v.plane + (long long)lj * d.v.pitch + li;
+    }
+    CK(cudaMemcpyAsync(d.src_offset, off.data(), n * sizeof(long long), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+  }
+  CK(cudaMemcpyAsync(c->d_wav, wav, (size_t)n * len * 4, cudaMemcpyHostToDevice, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  c->nsrc = n; c->wlen = len;
+  return FDTD_OK;
+}
+
+int fdtd_step(fdtd_ctx* c, int32_t n) {
+  if (!c || n < 0) return FDTD_EINVAL;
+  for (int s = 0; s < n; ++s) {
+    int r;
+    if ((r = do_substep(c, 0))) return r;     // velocity sub-update
+    if ((r = do_substep(c, 1))) return r;     // pressure sub-update
+    if ((r = launch_inject(c))) return r;     // source (R14)
+  }
+  return FDTD_OK;
+}
+
+static int field_bases(fdtd_ctx* c, int which, std::vector<float*>& bases) {
+  if (which < 0 || which > 3) { set_err("bad field selector"); return FDTD_EINVAL; }
+  for (auto& d : c->doms) bases.push_back(d.v.f[which]);
+  return FDTD_OK;
+}
+
+int fdtd_get_field(fdtd_ctx* c, int32_t which, float* dst) {
+  if (!c || !dst) return FDTD_EINVAL;
+  std::vector<float*> b;
+  int r = field_bases(c, which, b);
+  return r ? r : copy_field(c, b.data(), dst, true, true);
+}
+
+int fdtd_set_field(fdtd_ctx* c, int32_t which, const float* src) {
+  if (!c || !src) return FDTD_EINVAL;
+  std::vector<float*> b;
+  int r = field_bases(c, which, b);
+  if (r) return r;
+  c->substeps_done = 0;                       // ghosts are written consistently: restart the exchange cadence
+  return copy_field(c, b.data(), const_cast<float*>(src), false, false);
+}
+
+int fdtd_get_field_box(fdtd_ctx* c, int32_t which, const int32_t lo[3], const int32_t size[3], float* dst) {
+  if (!c || !lo || !size || !dst || which < 0 || which > 3) return FDTD_EINVAL;
+  for (int a = 0; a < 3; ++a)
+    if (lo[a] < 0 || size[a] <= 0 || lo[a] + size[a] > c->G.gn[a]) { set_err("box outside the grid"); return FDTD_EINVAL; }
+  for (auto& d : c->doms) {
+    const DomainView& v = d.v;
+    // intersection of the box with this domain's owned cells, in global coordinates
+    int g0[3], g1[3];
+    const int o[3] = {v.ox, v.oy, v.oz};
+    bool empty = false;
+    for (int a = 0; a < 3; ++a) {
+      g0[a] = std::max(lo[a], o[a] + d.own_lo[a]);
+      g1[a] = std::min(lo[a] + size[a], o[a] + d.own_hi[a]);
+      if (g1[a] <= g0[a]) empty = true;
+    }
+    if (empty) continue;
+    for (int gk = g0[2]; gk < g1[2]; ++gk) {
+      const float* dev = v.f[which] + (long long)(gk - v.oz) * v.plane + (long long)(g0[1] - v.oy) * v.pitch + (g0[0] - v.ox);
+      float* h = dst + ((long long)(gk - lo[2]) * size[1] + (g0[1] - lo[1])) * size[0] + (g0[0] - lo[0]);
+      CK(cudaMemcpy2DAsync(h, (size_t)size[0] * 4, dev, (size_t)v.pitch * 4, (size_t)(g1[0] - g0[0]) * 4, g1[1] - g0[1],
+                           cudaMemcpyDeviceToHost, c->stream));
+    }
+  }
+  CK(cudaStreamSynchronize(c->stream));
+  return FDTD_OK;
+}
+
+int fdtd_fill_hash(fdtd_ctx* c, int32_t which, uint64_t seed, double scale) {
+  if (!c || which < 0 || which > 3) return FDTD_EINVAL;
+  for (auto& d : c->doms) {
+    fill_hash_kernel<<<148 * 8, 256, 0, c->stream>>>(d.v, which, seed, (float)scale);
+    c->launches++;
+  }
+  c->substeps_done = 0;
+  CK(cudaGetLastError());
+  return FDTD_OK;
+}
+
+int fdtd_field_absmax(fdtd_ctx* c, int32_t which, const int32_t lo[3], const int32_t size[3], float* out) {
+  if (!c || !lo || !size || !out || which < 0 || which > 3) return FDTD_EINVAL;
+  for (int a = 0; a < 3; ++a)
+    if (lo[a] < 0 || size[a] <= 0 || lo[a] + size[a] > c->G.gn[a]) { set_err("box outside the grid"); return FDTD_EINVAL; }
+  unsigned int* acc = (unsigned int*)(c->ws + c->L.absmax);
+  CK(cudaMemsetAsync(acc, 0, 4, c->stream));
+  for (auto& d : c->doms) {
+    const DomainView& v = d.v;
+    const int o[3] = {v.ox, v.oy, v.oz};
+    int g0[3], g1[3];
+    bool empty = false;
+    for (int a = 0; a < 3; ++a) {
+      g0[a] = std::max(lo[a], o[a] + d.own_lo[a]);
+      g1[a] = std::min(lo[a] + size[a], o[a] + d.own_hi[a]);
+      if (g1[a] <= g0[a]) empty = true;
+    }
+    if (empty) continue;
+    absmax_kernel<<<148 * 4, 256, 0, c->stream>>>(v, which, g0[0] - o[0], g0[1] - o[1], g0[2] - o[2], g1[0] - g0[0], g1[1] - g0[1],
+                                                  g1[2] - g0[2], acc);
+    c->launches++;
+  }
+  CK(cudaGetLastError());
+  unsigned int bits = 0;
+  CK(cudaMemcpyAsync(&bits, acc, 4, cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  memcpy(out, &bits, 4);
+  return FDTD_OK;
+}
+
+int fdtd_get_psi(fdtd_ctx* c, int32_t which, float* dst) {
+  if (!c || !dst || which < 0 || which > 5) return FDTD_EINVAL;
+  const int fam = which / 3, axis = which % 3;
+  const int gnx = c->G.gn[0], gny = c->G.gn[1];
+  for (auto& d : c->doms) {
+    const DomainView& v = d.v;
+    const size_t n = (size_t)v.nx * v.ny * v.nz;
+    float* tmp = nullptr;
+    CK(cudaMalloc(&tmp, n * 4));                       // debug-only scratch, not field storage
+    expand_psi_kernel<<<148 * 8, 256, 0, c->stream>>>(v, fam, axis, tmp);
+    c->launches++;
+    for (int k = d.own_lo[2]; k < d.own_hi[2]; ++k) {
+      const float* dev = tmp + ((size_t)k * v.ny + d.own_lo[1]) * v.nx;
+      float* h = dst + ((size_t)(k + v.oz) * gny + (d.own_lo[1] + v.oy)) * gnx;
+      cudaMemcpyAsync(h, dev, (size_t)v.nx * (d.own_hi[1] - d.own_lo[1]) * 4, cudaMemcpyDeviceToHost, c->stream);
+    }
+    cudaError_t e = cudaStreamSynchronize(c->stream);
+    cudaFree(tmp);
+    CK(e);
+  }
+  return FDTD_OK;
+}
+
+int fdtd_cpml_table(fdtd_ctx* c, int32_t axis, int32_t half, float* a, float* b, float* ik) {
+  if (!c || axis < 0 || axis > 2 || !a || !b || !ik) return FDTD_EINVAL;
+  const AxisTable& t = c->tabs[half ? 0 : 1][axis];
+  const size_t n = (size_t)c->G.gn[axis];
+  memcpy(a, t.a.data(), n * 4); memcpy(b, t.b.data(), n * 4); memcpy(ik, t.ik.data(), n * 4);
+  return FDTD_OK;
+}
+
+int fdtd_destroy(fdtd_ctx* c) {
+  if (!c) return FDTD_EINVAL;
+  cudaError_t e = cudaStreamSynchronize(c->stream);
+  delete c;
+  if (e != cudaSuccess) { set_err(std::string("cudaStreamSynchronize: ") + cudaGetErrorString(e)); return FDTD_ECUDA; }
+  return FDTD_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,177 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Tolerance (BASELINE.json north_star, reading R17): max|delta| / max|oracle| <= 1e-4 per field, fp32.  The fp64 oracle
+(fed the same fp32 inputs) arbitrates (R18): the GPU and the fp32 oracle must each be within 1e-4 of it."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from oracle import Oracle
+from paper_2606_06910_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-4
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2606_06910_b200 import binding
+    return binding
+
+
+def rel(a, b):
+    s = np.abs(b).max()
+    return float(np.abs(a.astype(np.float64) - b).max() / (s if s > 0 else 1.0))
+
+
+def oracle_for(w, fp64=False):
+    o = Oracle(w.n_interior, w.cpml, fp64=fp64, **w.cpml_kwargs())
+    if w.c is not None:
+        o.set_model(w.c)
+    o.set_sources(w.sources, w.wavelets)
+    return o
+
+
+def test_coefficients_and_cpml_tables_match_oracle(B):
+    assert np.array_equal(B.fdtd_coeffs().view(np.uint32), oracle.coeffs().view(np.uint32))
+    w = inputs.config(1)
+    sim = B.from_workload(w)
+    o = oracle_for(w)
+    for axis in range(3):
+        for half in (0, 1):
+            a, b, ik = sim.cpml_table(axis, half)
+            oa, ob, oik, oin = o.cpml_table(axis, half)
+            assert np.array_equal(a, oa) and np.array_equal(b, ob) and np.array_equal(ik, oik)
+    sim.destroy()
+
+
+@pytest.mark.parametrize("kernel", [1, 0])
+def test_config1_full_parity(B, kernel):
+    """BASELINE config 1 in full: 64^3 + 8-cell CPML, centre Ricker source, 100 steps, zero initial fields."""
+    w = inputs.config(1)
+    sim = B.from_workload(w, kernel=kernel)
+    sim.step(w.steps)
+    o32, o64 = oracle_for(w), oracle_for(w, fp64=True)
+    o32.step(w.steps)
+    o64.step(w.steps)
+    for f in range(4):
+        g, r32, r64 = sim.get_field(f), o32.get(f), o64.get(f)
+        assert rel(g, r32) <= TOL, (f, rel(g, r32))
+        assert rel(g, r64) <= TOL and rel(r32, r64) <= TOL
+    for q in range(6):
+        g, r = sim.get_psi(q), o32.get(4 + q)
+        assert rel(g, r) <= TOL, (q, rel(g, r))
+    assert sim.launch_count() >= 2 * w.steps
+    sim.destroy()
+
+
+@pytest.mark.parametrize("kernel", [1, 0])
+@pytest.mark.parametrize("shape,cpml", [
+    ((70, 45, 37), (5, 9, 0, 7, 6, 0)),        # ragged tiles in x and y, faces without a layer, unequal thickness
+    ((133, 18, 21), (12, 12, 4, 4, 8, 8)),     # more than two x tiles, nx not a multiple of 4
+    ((24, 20, 150), (0, 0, 0, 0, 10, 10)),     # long in z: several z chunks
+])
+def test_random_state_ragged_parity(B, kernel, shape, cpml):
+    """All four fields random (counter-based generator on both sides), heterogeneous c, 6 steps."""
+    tot = tuple(shape[a] + cpml[2 * a] + cpml[2 * a + 1] for a in range(3))
+    rng = np.random.default_rng(11)
+    c = (1.0 + 0.3 * rng.random(tot[::-1])).astype(np.float32)
+    kw = dict(dt=0.4 / 1.3, cpml_alpha_max=math.pi * inputs.F0, cpml_c_ref=1.3)
+    sim = B.Fdtd(shape, cpml, kernel=kernel, **kw)
+    o = Oracle(shape, cpml, **kw)
+    sim.set_model(c)
+    o.set_model(c)
+    src = np.array([[tot[0] // 2, tot[1] // 3, tot[2] // 2], [3, 2, 1]], np.int32)
+    wav = np.stack([inputs.ricker(6, kw["dt"], t0=1.0), 0.1 * np.ones(6, np.float32)])
+    sim.set_sources(src, wav)
+    o.set_sources(src, wav)
+    for f in range(4):
+        sim.fill_hash(f, 42, 0.5)
+        o.fill_hash(f, 42, scale=0.5)
+    for f in range(4):                               # the two generators agree bit for bit
+        assert np.array_equal(sim.get_field(f), o.get(f).astype(np.float32)), f
+    sim.step(6)
+    o.step(6)
+    for f in range(4):
+        assert rel(sim.get_field(f), o.get(f)) <= TOL, (f, rel(sim.get_field(f), o.get(f)))
+    for q in range(6):
+        assert rel(sim.get_psi(q), o.get(4 + q)) <= TOL, q
+    sim.destroy()
+
+
+def test_tiled_and_reference_kernels_agree_bitwise(B):
+    shape, cpml = (90, 40, 33), (8, 8, 8, 8, 8, 8)
+    kw = dict(dt=0.4, cpml_alpha_max=math.pi * inputs.F0)
+    out = []
+    for kernel in (0, 1):
+        sim = B.Fdtd(shape, cpml, kernel=kernel, **kw)
+        for f in range(4):
+            sim.fill_hash(f, 7, 1.0)
+        sim.step(5)
+        out.append([sim.get_field(f) for f in range(4)] + [sim.get_psi(q) for q in range(6)])
+        sim.destroy()
+    for a, b in zip(*out):
+        assert np.array_equal(a, b)
+
+
+def test_periodic_dispersion_on_gpu(B):
+    """Pin P2 on the CUDA path (reference kernel, periodic): p^{n+1} + p^{n-1} = (2 - 4S) p^n."""
+    N, mode = 16, (1, 2, 3)
+    c = B.fdtd_coeffs().astype(np.float64)
+    nu = float(np.float32(0.4))
+    S = nu * nu * sum(sum(c[l] * math.sin((2 * l + 1) * math.pi * m / N) for l in range(4)) ** 2 for m in mode)
+    sim = B.Fdtd((N,) * 3, boundary=B.FDTD_PERIODIC, dt=0.4)
+    z, y, x = np.meshgrid(*(np.arange(N),) * 3, indexing="ij")
+    p0 = np.cos(2 * math.pi * (mode[0] * x + mode[1] * y + mode[2] * z) / N + 0.3).astype(np.float32)
+    sim.set_field(B.FDTD_P, p0)
+    hist = [p0.astype(np.float64)]
+    for _ in range(5):
+        sim.step(1)
+        hist.append(sim.get_field(B.FDTD_P).astype(np.float64))
+    for n in range(1, 5):
+        assert np.abs(hist[n + 1] + hist[n - 1] - (2 - 4 * S) * hist[n]).max() < 2e-6
+    sim.destroy()
+
+
+def test_cpml_reduces_to_interior_on_gpu(B):
+    """P:52 on the CUDA path: sigma = alpha = 0, kappa = 1 gives the same fields as the layer-free run."""
+    kw = dict(dt=0.4)
+    a = B.Fdtd((50, 30, 20), (7,) * 6, cpml_R0=1.0, cpml_alpha_max=0.0, **kw)
+    b = B.Fdtd((64, 44, 34), (0,) * 6, **kw)
+    for sim in (a, b):
+        for f in range(4):
+            sim.fill_hash(f, 3, 1.0)
+        sim.step(8)
+    for f in range(4):
+        assert np.array_equal(a.get_field(f), b.get_field(f))      # float equality: -0 == +0
+    for q in range(6):
+        assert not a.get_psi(q).any()
+    a.destroy()
+    b.destroy()
+
+
+def test_get_field_box_and_absmax(B):
+    sim = B.Fdtd((40, 30, 20), dt=0.4)
+    sim.fill_hash(B.FDTD_VY, 5, 2.0)
+    full = sim.get_field(B.FDTD_VY)
+    box = sim.get_field_box(B.FDTD_VY, (3, 4, 5), (17, 11, 7))
+    assert np.array_equal(box, full[5:12, 4:15, 3:20])
+    assert sim.field_absmax(B.FDTD_VY) == np.abs(full).max()
+    assert sim.field_absmax(B.FDTD_VY, (3, 4, 5), (17, 11, 7)) == np.abs(box).max()
+    sim.destroy()
+
+
+def test_errors_are_reported_not_fatal(B):
+    sim = B.Fdtd((16,) * 3, dt=0.4)
+    with pytest.raises(B.FdtdError):
+        sim.set_sources([(99, 0, 0)], np.zeros((1, 4), np.float32))
+    rho = np.ones(sim.shape, np.float32)
+    rho[0, 0, 0] = 2
+    with pytest.raises(B.FdtdError):
+        sim.set_model(None, rho)
+    sim.step(1)
+    sim.destroy()
