@@ -94,6 +94,11 @@ int fdtd_set_sources(fdtd_ctx* ctx, int32_t n, const int32_t* ijk_host, const fl
  * Asynchronous on params.stream; no host synchronisation. */
 int fdtd_step(fdtd_ctx* ctx, int32_t n);
 
+/* fdtd_step with CUDA events recorded on params.stream around every launch group: out_ms_host[0] = total time of
+ * the velocity sub-update kernels, [1] = pressure sub-update kernels, [2] = source injection, [3] = halo exchange,
+ * in milliseconds over the n steps.  Same arithmetic and launches as fdtd_step.  Synchronises. */
+int fdtd_step_profiled(fdtd_ctx* ctx, int32_t n, double out_ms_host[4]);
+
 /* Copies one field (FDTD_P..FDTD_VZ) of the total grid, unpadded, to dst_host (Nz*Ny*Nx fp32).  In subdomain
  * mode the owned cells of every subdomain are gathered.  Synchronises the stream. */
 int fdtd_get_field(fdtd_ctx* ctx, int32_t which, float* dst_host);

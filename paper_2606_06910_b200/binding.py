@@ -20,7 +20,7 @@ FDTD_OK, FDTD_EINVAL, FDTD_EWORKSPACE, FDTD_ECUDA, FDTD_EUNSUPPORTED = 0, -1, -2
 
 # every symbol include/fdtd_b200.h declares
 EXPORTS = [
-    "fdtd_workspace_bytes", "fdtd_create", "fdtd_set_model", "fdtd_set_sources", "fdtd_step", "fdtd_get_field",
+    "fdtd_workspace_bytes", "fdtd_create", "fdtd_set_model", "fdtd_set_sources", "fdtd_step", "fdtd_step_profiled", "fdtd_get_field",
     "fdtd_get_field_box", "fdtd_set_field", "fdtd_fill_hash", "fdtd_get_psi", "fdtd_field_absmax", "fdtd_cpml_table",
     "fdtd_coeffs", "fdtd_launch_count", "fdtd_dims", "fdtd_destroy", "fdtd_last_error",
 ]
@@ -66,6 +66,7 @@ def _load():
     L.fdtd_set_model.argtypes = [vp, vp, vp]
     L.fdtd_set_sources.argtypes = [vp, i32, vp, vp, i32]
     L.fdtd_step.argtypes = [vp, i32]
+    L.fdtd_step_profiled.argtypes = [vp, i32, vp]
     L.fdtd_get_field.argtypes = [vp, i32, vp]
     L.fdtd_get_field_box.argtypes = [vp, i32, vp, vp, vp]
     L.fdtd_set_field.argtypes = [vp, i32, vp]
@@ -163,6 +164,12 @@ class Fdtd:
 
     def step(self, n=1):
         _check(lib.fdtd_step(self._h, int(n)), "fdtd_step")
+
+    def step_profiled(self, n=1):
+        """-> dict of milliseconds per launch group over the n steps (CUDA events on the launching stream)."""
+        out = np.zeros(4, np.float64)
+        _check(lib.fdtd_step_profiled(self._h, int(n), out.ctypes.data), "fdtd_step_profiled")
+        return dict(update_v=float(out[0]), update_p=float(out[1]), inject=float(out[2]), exchange=float(out[3]))
 
     def get_field(self, which, out=None):
         if out is None:

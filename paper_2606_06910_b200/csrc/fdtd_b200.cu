@@ -418,6 +418,15 @@ int copy_field(fdtd_ctx* c, float* const* dom_base, float* host, bool to_host, b
     const int jl = owned_only ? d.own_lo[1] : 0, jh = owned_only ? d.own_hi[1] : v.ny;
     const int kl = owned_only ? d.own_lo[2] : 0, kh = owned_only ? d.own_hi[2] : v.nz;
     float* base = dom_base[&d - &c->doms[0]];
+    if (jl == 0 && jh == v.ny && v.ny == gny && v.oy == 0) {
+      // whole planes: rows of consecutive planes are consecutive on both sides -> one 2-D copy
+      float* dev = base + (long long)kl * v.plane;
+      float* h = host + (long long)(kl + v.oz) * gny * gnx;
+      const size_t rows = (size_t)(kh - kl) * v.ny;
+      if (to_host) CK(cudaMemcpy2DAsync(h, (size_t)gnx * 4, dev, (size_t)v.pitch * 4, (size_t)v.nx * 4, rows, cudaMemcpyDeviceToHost, c->stream));
+      else CK(cudaMemcpy2DAsync(dev, (size_t)v.pitch * 4, h, (size_t)gnx * 4, (size_t)v.nx * 4, rows, cudaMemcpyHostToDevice, c->stream));
+      continue;
+    }
     for (int k = kl; k < kh; ++k) {
       float* dev = base + (long long)k * v.plane + (long long)jl * v.pitch;
       float* h = host + ((long long)(k + v.oz) * gny + (jl + v.oy)) * gnx;
@@ -568,16 +577,23 @@ int fdtd_set_model(fdtd_ctx* c, const float* c_host, const float* rho_host) {
     for (auto& d : c->doms) { d.v.kc = nullptr; d.v.kc0 = (float)(rho * 1.0 * 1.0 * c->P.dt / c->P.dx); d.v.b0 = b0; }
     return FDTD_OK;
   }
-  std::vector<float> kc(n);
-  for (size_t q = 0; q < n; ++q) {
-    const double cc = c_host[q];
-    if (!(cc > 0.0)) { set_err("c must be positive"); return FDTD_EINVAL; }
-    kc[q] = (float)(rho * cc * cc * c->P.dt / c->P.dx);     // K dt/dx = rho c^2 dt/dx (R6), rounded once
-  }
+  // c goes up as fp32; K dt/dx = rho c^2 dt/dx (R6) is formed on the device in double and rounded once
   std::vector<float*> bases;
   for (size_t k = 0; k < c->doms.size(); ++k) bases.push_back((float*)(c->ws + c->L.doms[k].kc));
-  int r = copy_field(c, bases.data(), kc.data(), false, false);
+  int r = copy_field(c, bases.data(), const_cast<float*>(c_host), false, false);
   if (r) return r;
+  int* bad = (int*)(c->ws + c->L.absmax) + 4;
+  CK(cudaMemsetAsync(bad, 0, 4, c->stream));
+  for (size_t k = 0; k < c->doms.size(); ++k) {
+    const DomainView& v = c->doms[k].v;
+    speed_to_kc_kernel<<<148 * 8, 256, 0, c->stream>>>(bases[k], (long long)v.plane * v.nz, v.pitch, v.nx, rho, c->P.dt, c->P.dx, bad);
+    c->launches++;
+  }
+  CK(cudaGetLastError());
+  int nbad = 0;
+  CK(cudaMemcpyAsync(&nbad, bad, 4, cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  if (nbad) { set_err("c must be positive and finite"); return FDTD_EINVAL; }
   for (size_t k = 0; k < c->doms.size(); ++k) { c->doms[k].v.kc = bases[k]; c->doms[k].v.b0 = b0; }
   return FDTD_OK;
 }
@@ -614,6 +630,46 @@ int fdtd_step(fdtd_ctx* c, int32_t n) {
     if ((r = launch_inject(c))) return r;     // source (R14)
   }
   return FDTD_OK;
+}
+
+int fdtd_step_profiled(fdtd_ctx* c, int32_t n, double out_ms[4]) {
+  if (!c || n < 0 || !out_ms) return FDTD_EINVAL;
+  // One CUDA event on the launching stream after every launch group; the interval that ends at a mark is
+  // charged to the mark's category (0 = update_v, 1 = update_p, 2 = inject, 3 = exchange).
+  std::vector<cudaEvent_t> ev;
+  std::vector<int> cat;
+  int r = FDTD_OK;
+  auto mark = [&](int category) -> int {
+    cudaEvent_t e;
+    CK(cudaEventCreate(&e));
+    CK(cudaEventRecord(e, c->stream));
+    ev.push_back(e); cat.push_back(category);
+    return FDTD_OK;
+  };
+  r = mark(-1);
+  for (int s = 0; s < n && !r; ++s) {
+    for (int which = 0; which < 2 && !r; ++which) {
+      if (c->doms.size() > 1 && c->substeps_done % c->G.msub == 0) {
+        r = exchange_halos(c);
+        if (!r) r = mark(3);
+      }
+      for (auto& d : c->doms) if (!r) r = launch_substep(c, d, which);
+      c->substeps_done++;
+      if (!r) r = mark(which);
+    }
+    if (!r && c->nsrc > 0) { r = launch_inject(c); if (!r) r = mark(2); }
+  }
+  cudaError_t se = cudaStreamSynchronize(c->stream);
+  out_ms[0] = out_ms[1] = out_ms[2] = out_ms[3] = 0.0;
+  if (!r && se == cudaSuccess)
+    for (size_t k = 1; k < ev.size(); ++k) {
+      float ms = 0.f;
+      cudaEventElapsedTime(&ms, ev[k - 1], ev[k]);
+      out_ms[cat[k]] += ms;
+    }
+  for (auto& e : ev) cudaEventDestroy(e);
+  CK(se);
+  return r;
 }
 
 static int field_bases(fdtd_ctx* c, int which, std::vector<float*>& bases) {

@@ -490,6 +490,16 @@ __global__ void inject_sources(SourceView S, int advance) {
   if (advance && threadIdx.x == 0) *S.step = n + 1;
 }
 
+// In place: wave speed c (fp32) -> K dt/dx = rho c^2 dt/dx in double, rounded once to fp32 (R6).  Padding columns stay 0.
+__global__ void speed_to_kc_kernel(float* a, long long n, int pitch, int nx, double rho, double dt, double dx, int* bad) {
+  for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
+    if ((int)(t % pitch) >= nx) { a[t] = 0.f; continue; }
+    const double c = (double)a[t];
+    if (!(c > 0.0) || c > 1e30) atomicAdd(bad, 1);
+    a[t] = (float)(rho * c * c * dt / dx);
+  }
+}
+
 __device__ __forceinline__ uint64_t splitmix64(uint64_t x) {
   x += 0x9E3779B97F4A7C15ull;
   x = (x ^ (x >> 30)) * 0xBF58476D1CE4E5B9ull;
