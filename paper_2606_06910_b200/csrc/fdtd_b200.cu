@@ -116,7 +116,9 @@ struct Domain {
   DomainView v;
   int own_lo[3], own_hi[3];    // owned cells in local indices
   int cy, cz;                  // position in the subdomain grid
-  CUtensorMap tm_p, tm_vy;
+  TMaps tm;
+  unsigned int* counters = nullptr;  // device: [0] update_v work counter, [1] update_p work counter
+  Sched sched;
   long long* src_offset = nullptr;   // device, per source
 };
 
@@ -125,7 +127,7 @@ struct Layout {
   struct Dom {
     int n[3], o[3], pitch;
     int ls[3][2], ln[3][2];
-    uint64_t f[4], kc, psi[2][3][2], src_off;
+    uint64_t f[4], kc, psi[2][3][2], src_off, counters;
   };
   std::vector<Dom> doms;
   uint64_t tab[2][3][3];
@@ -171,6 +173,7 @@ Layout make_layout(const fdtd_params& P, const Geometry& G) {
           d.psi[fam][2][s] = take((uint64_t)d.pitch * d.n[1] * d.ln[2][s] * 4 + 16);
         }
       d.src_off = take(MAX_SRC * sizeof(long long));
+      d.counters = take(64);
       L.doms.push_back(d);
     }
   for (int a = 0; a < 3; ++a) {
@@ -216,8 +219,7 @@ struct fdtd_ctx {
   float* d_wav;
   int64_t launches = 0;
   int64_t substeps_done = 0;    // sub-updates since the last halo exchange (subdomain mode)
-  int zchunk_v = 0, zchunk_p = 0;
-  int nchunk_v = 1, nchunk_p = 1;
+  int grid_v = 0, grid_p = 0;       // resident CTAs of the whole GPU for each tiled kernel
 };
 
 namespace {
@@ -233,23 +235,31 @@ int make_tmap(EncodeTiledFn enc, CUtensorMap* m, float* base, const DomainView& 
   return FDTD_OK;
 }
 
-int pick_chunks(fdtd_ctx* c, const void* kernel, int smem, int nz, int tiles_xy, int* zchunk, int* nchunk) {
-  int per_sm = 0, dev = c->P.device, sms = 148;
+// Persistent launch plan: grid = resident CTAs; items = tiles x z-chunks with enough items per CTA for balance.
+int plan_launch(fdtd_ctx* c, const void* kernel, int smem, int* grid) {
+  int per_sm = 0, sms = 148;
   CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, NT, smem));
-  CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-  const long long cap = (long long)std::max(per_sm, 1) * sms;
-  int n;
-  if (const char* e = getenv("FDTD_ZCHUNK")) {
-    n = std::max(1, (nz + atoi(e) - 1) / std::max(1, atoi(e)));
-  } else if (tiles_xy >= cap) {
-    n = std::max(1, (nz + 127) / 128);                 // many waves: short chunks keep the tail small
-  } else {
-    n = (int)std::max(1LL, cap / tiles_xy);            // one wave: as many equal chunks as fit
-    n = std::min(n, std::max(1, nz / 8));
-  }
-  *zchunk = (nz + n - 1) / n;
-  *nchunk = (nz + *zchunk - 1) / *zchunk;
+  CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->P.device));
+  if (per_sm < 1) { set_err("tiled kernel does not fit on an SM"); return FDTD_ECUDA; }
+  if (const char* e = getenv("FDTD_CTAS_PER_SM")) per_sm = std::max(1, std::min(per_sm, atoi(e)));
+  *grid = per_sm * sms;
   return FDTD_OK;
+}
+
+void plan_items(Domain& d, int grid) {
+  const DomainView& v = d.v;
+  Sched& S = d.sched;
+  S.ntx = (v.nx + TX - 1) / TX;
+  S.nty = (v.ny + TY - 1) / TY;
+  const long long tiles = (long long)S.ntx * S.nty;
+  // about 8 items per resident CTA, chunks of 16..64 planes (each chunk re-reads 7 planes of the z-halo operand)
+  long long zc = (long long)v.nz * tiles / (8LL * std::max(grid, 1));
+  zc = std::max(16LL, std::min(64LL, zc));
+  if (const char* e = getenv("FDTD_ZCHUNK")) zc = std::max(1, atoi(e));
+  int n = (int)((v.nz + zc - 1) / zc);
+  S.zchunk = (v.nz + n - 1) / n;
+  S.nzc = (v.nz + S.zchunk - 1) / S.zchunk;
+  S.nitems = (int)(tiles * S.nzc);
 }
 
 int launch_substep(fdtd_ctx* c, Domain& d, int which /*0 = v, 1 = p*/) {
@@ -259,9 +269,11 @@ int launch_substep(fdtd_ctx* c, Domain& d, int which /*0 = v, 1 = p*/) {
     if (which == 0) update_v_ref<<<g, b, 0, c->stream>>>(v);
     else update_p_ref<<<g, b, 0, c->stream>>>(v);
   } else {
-    dim3 g((v.nx + TX - 1) / TX, (v.ny + TY - 1) / TY, which == 0 ? c->nchunk_v : c->nchunk_p);
-    if (which == 0) update_v_tiled<<<g, NT, V_SMEM_BYTES, c->stream>>>(d.tm_p, v, c->zchunk_v);
-    else update_p_tiled<<<g, NT, P_SMEM_BYTES, c->stream>>>(d.tm_vy, v, c->zchunk_p);
+    Sched S = d.sched;
+    S.counter = d.counters + which;
+    S.other = d.counters + (1 - which);
+    if (which == 0) update_v_tiled<<<std::min(c->grid_v, S.nitems), NT, V_SMEM_BYTES, c->stream>>>(d.tm, v, S);
+    else update_p_tiled<<<std::min(c->grid_p, S.nitems), NT, P_SMEM_BYTES, c->stream>>>(d.tm, v, S);
   }
   c->launches++;
   CK(cudaGetLastError());
@@ -535,8 +547,14 @@ fdtd_ctx* fdtd_create(const fdtd_params* P) {
         d.own_hi[a] = d.own_lo[a] + G.gn[a] / G.nd[a];
       }
       d.src_offset = (long long*)(c->ws + ld.src_off);
+      d.counters = (unsigned int*)(c->ws + ld.counters);
       if (!c->use_ref) {
-        if (make_tmap(enc, &d.tm_p, v.f[0], v, VW, VH) || make_tmap(enc, &d.tm_vy, v.f[2], v, PW, PH)) { delete c; return nullptr; }
+        float* kcbase = (float*)(c->ws + ld.kc);
+        float* tile_base[5] = {v.f[0], v.f[1], v.f[2], v.f[3], kcbase};
+        int bad = make_tmap(enc, &d.tm.p_halo, v.f[0], v, HW, VH) || make_tmap(enc, &d.tm.vx_halo, v.f[1], v, HW, TY) ||
+                  make_tmap(enc, &d.tm.vy_halo, v.f[2], v, TX, PH);
+        for (int t = 0; t < 5 && !bad; ++t) bad = make_tmap(enc, &d.tm.tile[t], tile_base[t], v, TX, TY);
+        if (bad) { delete c; return nullptr; }
       }
       c->doms.push_back(d);
     }
@@ -546,10 +564,9 @@ fdtd_ctx* fdtd_create(const fdtd_params* P) {
       return fail(c, e, "cudaFuncSetAttribute(update_v_tiled)");
     if ((e = cudaFuncSetAttribute(update_p_tiled, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM_BYTES)) != cudaSuccess)
       return fail(c, e, "cudaFuncSetAttribute(update_p_tiled)");
-    const DomainView& v0 = c->doms[0].v;
-    const int tiles = ((v0.nx + TX - 1) / TX) * ((v0.ny + TY - 1) / TY);
-    if (pick_chunks(c, (const void*)update_v_tiled, V_SMEM_BYTES, v0.nz, tiles, &c->zchunk_v, &c->nchunk_v) ||
-        pick_chunks(c, (const void*)update_p_tiled, P_SMEM_BYTES, v0.nz, tiles, &c->zchunk_p, &c->nchunk_p)) { delete c; return nullptr; }
+    if (plan_launch(c, (const void*)update_v_tiled, V_SMEM_BYTES, &c->grid_v) ||
+        plan_launch(c, (const void*)update_p_tiled, P_SMEM_BYTES, &c->grid_p)) { delete c; return nullptr; }
+    for (auto& d : c->doms) plan_items(d, std::min(c->grid_v, c->grid_p));
   }
   return c;
 }

@@ -165,21 +165,48 @@ __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarr
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // ---------------------------------------------------------------- tiled kernels
-constexpr int TX = 64;            // tile width in x (floats); 16 lanes x V4
-constexpr int TY = 16;            // tile height in y (rows)
-constexpr int NT = 256;           // threads per CTA
-constexpr int VW = TX + 8;        // p tile for update_v: columns x0-4 .. x0+TX+3
-constexpr int VH = TY + 7;        //                      rows    y0-3 .. y0+TY+3
-constexpr int VSTAGES = 4;
-constexpr int PW = TX;            // vy tile for update_p: columns x0 .. x0+TX-1
-constexpr int PH = TY + 8;        //                       rows    y0-4 .. y0+TY+3
-constexpr int PSTAGES = 4;
-constexpr int V_TILE_BYTES = VW * VH * 4;                       // bytes one TMA box delivers
-constexpr int P_TILE_BYTES = PW * PH * 4;
-constexpr int V_STAGE_FLOATS = ((V_TILE_BYTES + 127) / 128) * 32;  // stage stride: TMA destinations stay 128-B aligned
-constexpr int P_STAGE_FLOATS = ((P_TILE_BYTES + 127) / 128) * 32;
-constexpr int V_SMEM_BYTES = VSTAGES * V_STAGE_FLOATS * 4;
-constexpr int P_SMEM_BYTES = PSTAGES * P_STAGE_FLOATS * 4;
+// Persistent CTAs (grid = resident CTAs of the whole GPU) pull work items from an atomic counter.  One item is a
+// 64x16 (x,y) tile over a chunk of z planes.  Every operand of an item arrives in shared memory through TMA into a
+// 3-stage ring (one mbarrier per stage, armed with the stage's byte count), so the streaming loads run ahead of the
+// arithmetic without holding registers; results leave through 128-bit stores.  z neighbours live in a register queue.
+// Items away from every boundary and CPML slab take a mask-free path; the others take the general path.
+constexpr int TX = 64;             // tile width in x (floats): 16 lanes x 4
+constexpr int TY = 16;             // tile height in y (rows)
+constexpr int NT = 256;            // threads per CTA
+constexpr int NS = 3;              // ring stages
+constexpr int HW = TX + 8;         // x-halo tile width: columns x0-4 .. x0+TX+3
+constexpr int VH = TY + 7;         // p rows for update_v: y0-3 .. y0+TY+3
+constexpr int PH = TY + 8;         // vy rows for update_p: y0-4 .. y0+TY+3
+constexpr int TILE_FLOATS = TX * TY;
+constexpr int TILE_BYTES = TILE_FLOATS * 4;
+// update_v stage: [p halo tile | vx | vy | vz]
+constexpr int V_P_BYTES = HW * VH * 4;
+constexpr int V_P_FLOATS = ((V_P_BYTES + 127) / 128) * 32;     // keep every TMA destination 128-B aligned
+constexpr int V_OFF_VX = V_P_FLOATS, V_OFF_VY = V_OFF_VX + TILE_FLOATS, V_OFF_VZ = V_OFF_VY + TILE_FLOATS;
+constexpr int V_STAGE_FLOATS = V_OFF_VZ + TILE_FLOATS;
+constexpr int V_SMEM_BYTES = NS * V_STAGE_FLOATS * 4;
+// update_p stage: [vx x-halo tile | vy y-halo tile | vz | p | kc]
+constexpr int P_VX_BYTES = HW * TY * 4;
+constexpr int P_VY_BYTES = TX * PH * 4;
+constexpr int P_OFF_VY = P_VX_BYTES / 4, P_OFF_VZ = P_OFF_VY + P_VY_BYTES / 4, P_OFF_P = P_OFF_VZ + TILE_FLOATS, P_OFF_KC = P_OFF_P + TILE_FLOATS;
+constexpr int P_STAGE_FLOATS = P_OFF_KC + TILE_FLOATS;
+constexpr int P_SMEM_BYTES = NS * P_STAGE_FLOATS * 4;
+static_assert(P_VX_BYTES % 128 == 0 && P_VY_BYTES % 128 == 0 && TILE_BYTES % 128 == 0, "TMA destinations must stay 128-B aligned");
+
+struct TMaps {
+  CUtensorMap p_halo;     // p,  box HW x VH   (update_v)
+  CUtensorMap vx_halo;    // vx, box HW x TY   (update_p)
+  CUtensorMap vy_halo;    // vy, box TX x PH   (update_p)
+  CUtensorMap tile[5];    // p, vx, vy, vz, kc with box TX x TY
+};
+
+// Work decomposition of one launch (same for both sub-updates of a domain).
+struct Sched {
+  int ntx, nty, nzc, zchunk;   // tiles in x, y; chunks in z; planes per chunk
+  int nitems;
+  unsigned int* counter;       // this launch's work counter
+  unsigned int* other;         // the counter of the next launch on this domain: reset here
+};
 
 // Four consecutive x values held in registers; moved as one 128-bit access.
 struct V4 { float v[4]; };
@@ -191,286 +218,353 @@ __device__ __forceinline__ V4 splat4(float x) { V4 r; r.v[0] = r.v[1] = r.v[2] =
 __device__ __forceinline__ V4 zero4() { return splat4(0.f); }
 #define F4(a, e) ((a).v[e])
 
-// Velocity sub-update: v_a <- v_a - B [(1/kappa_a) D+_a p + psi_va] on planes [z0, z1) of one tile.
-// On arrival of p plane m: vx, vy of plane m are updated from the shared-memory tile, p[m] enters the register
-// queue, and vz of plane m-4 is updated from the queue (D+_z at k+1/2 reads p[k-3 .. k+4]).
-__global__ void __launch_bounds__(NT) update_v_tiled(const __grid_constant__ CUtensorMap tm_p, DomainView D, int zchunk) {
-  extern __shared__ __align__(128) unsigned char smem_raw[];
-  float* tiles = reinterpret_cast<float*>(smem_raw);
-  __shared__ __align__(8) uint64_t full[VSTAGES];
-
-  const int z0 = blockIdx.z * zchunk;
-  if (z0 >= D.nz) return;
-  const int z1 = min(z0 + zchunk, D.nz);
-  const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
-  const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
-  const int i = x0 + 4 * tx, j = y0 + ty;
-  const bool active = (i < D.nx) && (j < D.ny);
-  const int gj = j + D.oy;
-
-  if (threadIdx.x == 0) {
-#pragma unroll
-    for (int s = 0; s < VSTAGES; ++s) mbar_init(&full[s], 1);
-    fence_barrier_init();
-  }
-  __syncthreads();
-
-  const int m_begin = z0 - 3, m_end = z1 + 4;       // p planes m_begin .. m_end-1 are consumed
-  if (threadIdx.x == 0) {
-#pragma unroll
-    for (int s = 0; s < VSTAGES; ++s)
-      if (m_begin + s < m_end) {
-        mbar_expect_tx(&full[s], V_TILE_BYTES);
-        tma_load_3d(tiles + s * V_STAGE_FLOATS, &tm_p, &full[s], x0 - 4, y0 - 3, m_begin + s);
-      }
-  }
-
-  // per-thread invariants
-  const long long rowoff = (long long)j * D.pitch + i;
-  float* __restrict__ vx = D.f[1];
-  float* __restrict__ vy = D.f[2];
-  float* __restrict__ vz = D.f[3];
-  const float B = D.b0;
-  // keep-masks: component e is written only if it is a real column and not the pinned last half node (R3)
-  bool wx[4], wc[4];
+// D along x for four consecutive outputs from the 12 values w[n] = f[i-4+n]:
+//   FWD (D+ at i+e+1/2): f[i+e+l] - f[i+e-l+1];  BWD (D- at node i+e): f[i+e+l-1] - f[i+e-l]
+template <bool FWD>
+__device__ __forceinline__ V4 diff_x(const V4& l, const V4& c, const V4& r) {
+  const float w[12] = {l.v[0], l.v[1], l.v[2], l.v[3], c.v[0], c.v[1], c.v[2], c.v[3], r.v[0], r.v[1], r.v[2], r.v[3]};
+  V4 d;
 #pragma unroll
   for (int e = 0; e < 4; ++e) {
-    wc[e] = (i + e) < D.nx;
-    wx[e] = wc[e] && (D.periodic || (i + e + D.ox) != D.gn[0] - 1);
+    const int o = FWD ? 4 + e : 3 + e;   // index of the first "hi" operand minus 1
+    d.v[e] = stag_diff(w[o + 1], w[o], w[o + 2], w[o - 1], w[o + 3], w[o - 2], w[o + 4], w[o - 3]);
   }
-  const bool wy_row = gj != D.gn[1] - 1;
-  // CPML x / y slabs touched by this thread (x: the V4 lies wholly inside or outside a storage slab)
-  const int sx = active ? slab_side(D, 0, i) : -1;
-  const int sy = active ? slab_side(D, 1, j) : -1;
-  V4 ax = zero4(), bx = zero4(), ikx = zero4();
-  float ay = 0.f, by = 0.f, iky = 1.f;
-  if (sx >= 0) {
-    ax = ldg4(D.tab[0][0][0] + i + D.ox); bx = ldg4(D.tab[0][0][1] + i + D.ox); ikx = ldg4(D.tab[0][0][2] + i + D.ox);
+  return d;
+}
+__device__ __forceinline__ V4 diff_8(const V4& h1, const V4& l1, const V4& h2, const V4& l2, const V4& h3, const V4& l3, const V4& h4,
+                                     const V4& l4) {
+  V4 d;
+#pragma unroll
+  for (int e = 0; e < 4; ++e) d.v[e] = stag_diff(h1.v[e], l1.v[e], h2.v[e], l2.v[e], h3.v[e], l3.v[e], h4.v[e], l4.v[e]);
+  return d;
+}
+
+// ---- velocity sub-update: v_a <- v_a - B [(1/kappa_a) D+_a p + psi_va] for one item.
+// On arrival of stage "p plane m": vx, vy of plane m are updated from the tile, p[m] enters the register queue and
+// vz of plane m-4 is updated from the queue (D+_z at k+1/2 reads p[k-3 .. k+4]).
+template <bool EDGE>
+__device__ __forceinline__ void v_item(const TMaps& tm, const DomainView& D, float* smem, uint64_t* full, unsigned& it, int x0, int y0,
+                                       int z0, int z1) {
+  const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+  const int i = x0 + 4 * tx, j = y0 + ty;
+  const int m_begin = z0 - 3, m_end = z1 + 4;
+
+  auto issue = [&](unsigned slot, int m) {
+    const bool xy = m >= z0 && m < z1, zz = (m - 4) >= z0 && (m - 4) < z1;
+    uint64_t* bar = &full[slot];
+    float* st = smem + slot * V_STAGE_FLOATS;
+    mbar_expect_tx(bar, V_P_BYTES + (xy ? 2 * TILE_BYTES : 0) + (zz ? TILE_BYTES : 0));
+    tma_load_3d(st, &tm.p_halo, bar, x0 - 4, y0 - 3, m);
+    if (xy) {
+      tma_load_3d(st + V_OFF_VX, &tm.tile[1], bar, x0, y0, m);
+      tma_load_3d(st + V_OFF_VY, &tm.tile[2], bar, x0, y0, m);
+    }
+    if (zz) tma_load_3d(st + V_OFF_VZ, &tm.tile[3], bar, x0, y0, m - 4);
+  };
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < NS; ++s)
+      if (m_begin + s < m_end) issue((it + s) % NS, m_begin + s);
   }
-  if (sy >= 0) { ay = __ldg(D.tab[0][1][0] + gj); by = __ldg(D.tab[0][1][1] + gj); iky = __ldg(D.tab[0][1][2] + gj); }
+
+  const float B = D.b0;
+  const long long rowoff = (long long)j * D.pitch + i;
+  float* gvx = D.f[1] + rowoff + (long long)z0 * D.plane;
+  float* gvy = D.f[2] + rowoff + (long long)z0 * D.plane;
+  float* gvz = D.f[3] + rowoff + (long long)z0 * D.plane;
+  const int poff = (ty + 3) * HW + 4 * tx + 4;      // own float4 inside the p halo tile
+  const int toff = ty * TX + 4 * tx;                // own float4 inside a plain tile
+
+  // general path only: masks and CPML bookkeeping
+  bool active = true, wy_row = true;
+  bool wc[4] = {true, true, true, true}, wx[4] = {true, true, true, true};
+  int sx = -1, sy = -1;
+  if (EDGE) {
+    active = (i < D.nx) && (j < D.ny);
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      wc[e] = (i + e) < D.nx;                                         // real column (padding columns stay 0)
+      wx[e] = wc[e] && (i + e + D.ox) != D.gn[0] - 1;                 // not the pinned last half node (R3)
+    }
+    wy_row = (j + D.oy) != D.gn[1] - 1;
+    sx = active ? slab_side(D, 0, i) : -1;
+    sy = active ? slab_side(D, 1, j) : -1;
+  }
 
   V4 q0 = zero4(), q1 = zero4(), q2 = zero4(), q3 = zero4(), q4 = zero4(), q5 = zero4(), q6 = zero4(), q7 = zero4();
 
-  int it = 0;
   for (int m = m_begin; m < m_end; ++m, ++it) {
-    const int s = it % VSTAGES;
-    const uint32_t parity = (it / VSTAGES) & 1;
-    const bool do_xy = active && m >= z0 && m < z1;
+    const unsigned slot = it % NS;
+    const float* st = smem + slot * V_STAGE_FLOATS;
+    mbar_wait(&full[slot], (it / NS) & 1);
+    const bool xy = m >= z0 && m < z1;
     const int kz = m - 4;
-    const bool do_z = active && kz >= z0 && kz < z1 && (D.periodic || (kz + D.oz) != D.gn[2] - 1);
-    // issue the streaming loads before waiting on the tile
-    V4 vx4 = zero4(), vy4 = zero4(), vz4 = zero4(), psx = zero4(), psy = zero4(), psz = zero4();
-    const long long qxy = (long long)m * D.plane + rowoff;
-    const long long qz = (long long)kz * D.plane + rowoff;
-    int sz = -1;
-    if (do_xy) {
-      vx4 = ld4(vx + qxy);
-      vy4 = ld4(vy + qxy);
-      if (sx >= 0) psx = ld4(D.psi[0][0][sx] + psi_index(D, 0, sx, i, j, m));
-      if (sy >= 0) psy = ld4(D.psi[0][1][sy] + psi_index(D, 1, sy, i, j, m));
-    }
-    if (do_z) {
-      vz4 = ld4(vz + qz);
-      sz = slab_side(D, 2, kz);
-      if (sz >= 0) psz = ld4(D.psi[0][2][sz] + psi_index(D, 2, sz, i, j, kz));
-    }
+    const bool zz = kz >= z0 && kz < z1;
 
-    mbar_wait(&full[s], parity);
-    const float* row = tiles + s * V_STAGE_FLOATS + (ty + 3) * VW + 4 * tx + 4;
+    const float* row = st + poff;
     const V4 c = ld4(row);
-    V4 dxv, dyv;
-    {
-      const V4 l = ld4(row - 4), r = ld4(row + 4);
-      const float w[12] = {l.v[0], l.v[1], l.v[2], l.v[3], c.v[0], c.v[1], c.v[2], c.v[3], r.v[0], r.v[1], r.v[2], r.v[3]};   // p[i-4+n]
-#pragma unroll
-      for (int e = 0; e < 4; ++e)
-        F4(dxv, e) = stag_diff(w[5 + e], w[4 + e], w[6 + e], w[3 + e], w[7 + e], w[2 + e], w[8 + e], w[1 + e]);
-      const V4 yp1 = ld4(row + VW), yp2 = ld4(row + 2 * VW), yp3 = ld4(row + 3 * VW), yp4 = ld4(row + 4 * VW);
-      const V4 ym1 = ld4(row - VW), ym2 = ld4(row - 2 * VW), ym3 = ld4(row - 3 * VW);
-#pragma unroll
-      for (int e = 0; e < 4; ++e)
-        F4(dyv, e) = stag_diff(F4(yp1, e), F4(c, e), F4(yp2, e), F4(ym1, e), F4(yp3, e), F4(ym2, e), F4(yp4, e), F4(ym3, e));
+    V4 dxv, dyv, vx4, vy4, vz4;
+    if (xy) {
+      dxv = diff_x<true>(ld4(row - 4), c, ld4(row + 4));
+      dyv = diff_8(ld4(row + HW), c, ld4(row + 2 * HW), ld4(row - HW), ld4(row + 3 * HW), ld4(row - 2 * HW), ld4(row + 4 * HW),
+                   ld4(row - 3 * HW));
+      vx4 = ld4(st + V_OFF_VX + toff);
+      vy4 = ld4(st + V_OFF_VY + toff);
     }
-    q0 = q1; q1 = q2; q2 = q3; q3 = q4; q4 = q5; q5 = q6; q6 = q7; q7 = c;    // q7 = p[m], q0 = p[m-7]
-    __syncthreads();                                                            // every thread is done with stage s
-    if (threadIdx.x == 0 && m + VSTAGES < m_end) {
-      mbar_expect_tx(&full[s], V_TILE_BYTES);
-      tma_load_3d(tiles + s * V_STAGE_FLOATS, &tm_p, &full[s], x0 - 4, y0 - 3, m + VSTAGES);
-    }
+    if (zz) vz4 = ld4(st + V_OFF_VZ + toff);
+    q0 = q1; q1 = q2; q2 = q3; q3 = q4; q4 = q5; q5 = q6; q6 = q7; q7 = c;     // q7 = p[m] ... q0 = p[m-7]
+    __syncthreads();                                                             // every thread is done with this stage
+    if (tid == 0 && m + NS < m_end) issue(slot, m + NS);
 
-    if (do_xy) {
-      if (sx >= 0) {
+    if (xy) {
+      if (!EDGE) {
+#pragma unroll
+        for (int e = 0; e < 4; ++e) { vx4.v[e] = upd(vx4.v[e], B, dxv.v[e]); vy4.v[e] = upd(vy4.v[e], B, dyv.v[e]); }
+        st4(gvx, vx4);
+        st4(gvy, vy4);
+      } else if (active) {
+        if (sx >= 0) {
+          float* pp = D.psi[0][0][sx] + psi_index(D, 0, sx, i, j, m);
+          V4 ps = ld4(pp);
+          const V4 a = ldg4(D.tab[0][0][0] + i + D.ox), b = ldg4(D.tab[0][0][1] + i + D.ox), ik = ldg4(D.tab[0][0][2] + i + D.ox);
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const float old = ps.v[e];
+            dxv.v[e] = cpml_apply(dxv.v[e], ps.v[e], a.v[e], b.v[e], ik.v[e]);
+            if (!wx[e]) ps.v[e] = old;                                 // the pinned half node keeps its psi too
+          }
+          st4(pp, ps);
+        }
+        if (sy >= 0 && wy_row) {
+          float* pp = D.psi[0][1][sy] + psi_index(D, 1, sy, i, j, m);
+          V4 ps = ld4(pp);
+          const int gj = j + D.oy;
+          const float a = __ldg(D.tab[0][1][0] + gj), b = __ldg(D.tab[0][1][1] + gj), ik = __ldg(D.tab[0][1][2] + gj);
+#pragma unroll
+          for (int e = 0; e < 4; ++e) dyv.v[e] = cpml_apply(dyv.v[e], ps.v[e], a, b, ik);
+          st4(pp, ps);
+        }
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
-          const float old = F4(psx, e);
-          F4(dxv, e) = cpml_apply(F4(dxv, e), F4(psx, e), F4(ax, e), F4(bx, e), F4(ikx, e));
-          if (!wx[e]) F4(psx, e) = old;          // the pinned half node keeps its psi too (R3)
+          const float nvx = upd(vx4.v[e], B, dxv.v[e]), nvy = upd(vy4.v[e], B, dyv.v[e]);
+          vx4.v[e] = wx[e] ? nvx : (wc[e] ? vx4.v[e] : 0.f);
+          vy4.v[e] = wc[e] ? (wy_row ? nvy : vy4.v[e]) : 0.f;
         }
-        st4(D.psi[0][0][sx] + psi_index(D, 0, sx, i, j, m), psx);
+        st4(gvx, vx4);
+        st4(gvy, vy4);
       }
-      if (sy >= 0 && wy_row) {
-#pragma unroll
-        for (int e = 0; e < 4; ++e) F4(dyv, e) = cpml_apply(F4(dyv, e), F4(psy, e), ay, by, iky);
-        st4(D.psi[0][1][sy] + psi_index(D, 1, sy, i, j, m), psy);
-      }
-#pragma unroll
-      for (int e = 0; e < 4; ++e) {
-        const float nvx = upd(F4(vx4, e), B, F4(dxv, e));
-        F4(vx4, e) = wx[e] ? nvx : (wc[e] ? F4(vx4, e) : 0.f);
-        const float nvy = upd(F4(vy4, e), B, F4(dyv, e));
-        F4(vy4, e) = wc[e] ? ((D.periodic || wy_row) ? nvy : F4(vy4, e)) : 0.f;
-      }
-      st4(vx + qxy, vx4);
-      st4(vy + qxy, vy4);
+      gvx += D.plane;
+      gvy += D.plane;
     }
-    if (do_z) {
-      V4 dzv;
+    if (zz) {
+      // D+_z at kz+1/2: p[kz+l] = q(3+l), p[kz-l+1] = q(4-l)
+      V4 dzv = diff_8(q4, q3, q5, q2, q6, q1, q7, q0);
+      if (!EDGE) {
 #pragma unroll
-      for (int e = 0; e < 4; ++e)   // D+_z at kz+1/2: p[kz+l] = q(3+l), p[kz-l+1] = q(4-l)
-        F4(dzv, e) = stag_diff(F4(q4, e), F4(q3, e), F4(q5, e), F4(q2, e), F4(q6, e), F4(q1, e), F4(q7, e), F4(q0, e));
-      if (sz >= 0) {
-        const int gk = kz + D.oz;
-        const float az = __ldg(D.tab[0][2][0] + gk), bz = __ldg(D.tab[0][2][1] + gk), ikz = __ldg(D.tab[0][2][2] + gk);
+        for (int e = 0; e < 4; ++e) vz4.v[e] = upd(vz4.v[e], B, dzv.v[e]);
+        st4(gvz, vz4);
+      } else if (active && (kz + D.oz) != D.gn[2] - 1) {
+        const int sz = slab_side(D, 2, kz);
+        if (sz >= 0) {
+          float* pp = D.psi[0][2][sz] + psi_index(D, 2, sz, i, j, kz);
+          V4 ps = ld4(pp);
+          const int gk = kz + D.oz;
+          const float a = __ldg(D.tab[0][2][0] + gk), b = __ldg(D.tab[0][2][1] + gk), ik = __ldg(D.tab[0][2][2] + gk);
 #pragma unroll
-        for (int e = 0; e < 4; ++e) F4(dzv, e) = cpml_apply(F4(dzv, e), F4(psz, e), az, bz, ikz);
-        st4(D.psi[0][2][sz] + psi_index(D, 2, sz, i, j, kz), psz);
+          for (int e = 0; e < 4; ++e) dzv.v[e] = cpml_apply(dzv.v[e], ps.v[e], a, b, ik);
+          st4(pp, ps);
+        }
+#pragma unroll
+        for (int e = 0; e < 4; ++e) vz4.v[e] = wc[e] ? upd(vz4.v[e], B, dzv.v[e]) : 0.f;
+        st4(gvz, vz4);
       }
-#pragma unroll
-      for (int e = 0; e < 4; ++e) F4(vz4, e) = wc[e] ? upd(F4(vz4, e), B, F4(dzv, e)) : 0.f;
-      st4(vz + qz, vz4);
+      gvz += D.plane;
     }
   }
 }
 
-// Pressure sub-update: p <- p - Kc [sum_a (1/kappa_a) D-_a v_a + psi_pa] on planes [z0, z1).
-// vx: own V4 + left/right neighbours by 128-bit loads; vy: TMA-staged tile (rows y0-4 .. y0+TY+3);
-// vz: register queue along z (D-_z at node k reads vz[k-4 .. k+3]).
-__global__ void __launch_bounds__(NT) update_p_tiled(const __grid_constant__ CUtensorMap tm_vy, DomainView D, int zchunk) {
-  extern __shared__ __align__(128) unsigned char smem_raw[];
-  float* tiles = reinterpret_cast<float*>(smem_raw);
-  __shared__ __align__(8) uint64_t full[PSTAGES];
-
-  const int z0 = blockIdx.z * zchunk;
-  if (z0 >= D.nz) return;
-  const int z1 = min(z0 + zchunk, D.nz);
-  const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
-  const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
-  const int i = x0 + 4 * tx, j = y0 + ty;
-  const bool active = (i < D.nx) && (j < D.ny);
-  const int gj = j + D.oy;
-
-  if (threadIdx.x == 0) {
+// does the item [x0,x0+TX) x [y0,y0+TY) x [z0,z1) need masks or CPML code?
+__device__ __forceinline__ bool item_is_edge(const DomainView& D, int x0, int y0, int z0, int z1) {
+  if (x0 + TX >= D.nx || y0 + TY >= D.ny || z1 >= D.nz) return true;     // ragged tile or the pinned last index
+  const int lo[3] = {x0, y0, z0}, hi[3] = {x0 + TX, y0 + TY, z1};
 #pragma unroll
-    for (int s = 0; s < PSTAGES; ++s) mbar_init(&full[s], 1);
-    fence_barrier_init();
-  }
+  for (int a = 0; a < 3; ++a)
+#pragma unroll
+    for (int s = 0; s < 2; ++s)
+      if (D.ln[a][s] > 0 && lo[a] < D.ls[a][s] + D.ln[a][s] && hi[a] > D.ls[a][s]) return true;
+  return false;
+}
+
+__device__ __forceinline__ bool next_item(const Sched& S, int* s_item, int& x0, int& y0, int& z0, int& z1, int nz) {
+  __syncthreads();                                   // previous item fully consumed (smem tiles and s_item)
+  if (threadIdx.x == 0) *s_item = (int)atomicAdd(S.counter, 1u);
   __syncthreads();
+  const int item = *s_item;
+  if (item >= S.nitems) return false;
+  const int txi = item % S.ntx, r = item / S.ntx;
+  const int tyi = r % S.nty, zc = r / S.nty;
+  x0 = txi * TX; y0 = tyi * TY; z0 = zc * S.zchunk; z1 = min(z0 + S.zchunk, nz);
+  return true;
+}
+
+__global__ void __launch_bounds__(NT, 3) update_v_tiled(const __grid_constant__ TMaps tm, const __grid_constant__ DomainView D,
+                                                        const __grid_constant__ Sched S) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  float* smem = reinterpret_cast<float*>(smem_raw);
+  __shared__ __align__(8) uint64_t full[NS];
+  __shared__ int s_item;
   if (threadIdx.x == 0) {
 #pragma unroll
-    for (int s = 0; s < PSTAGES; ++s)
-      if (z0 + s < z1) {
-        mbar_expect_tx(&full[s], P_TILE_BYTES);
-        tma_load_3d(tiles + s * P_STAGE_FLOATS, &tm_vy, &full[s], x0, y0 - 4, z0 + s);
-      }
+    for (int s = 0; s < NS; ++s) mbar_init(&full[s], 1);
+    fence_barrier_init();
+    if (blockIdx.x == 0) *S.other = 0u;              // arm the next launch's work counter
+  }
+  unsigned it = 0;
+  int x0, y0, z0, z1;
+  while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) {
+    if (item_is_edge(D, x0, y0, z0, z1)) v_item<true>(tm, D, smem, full, it, x0, y0, z0, z1);
+    else v_item<false>(tm, D, smem, full, it, x0, y0, z0, z1);
+  }
+}
+
+// ---- pressure sub-update: p <- p - Kc [sum_a (1/kappa_a) D-_a v_a + psi_pa] for one item.
+// Stage "vz plane m" also carries vx (x-halo tile), vy (y-halo tile), p and Kc of plane k = m-3; vz[m] enters the
+// register queue and p[k] is updated (D-_z at node k reads vz[k-4 .. k+3]).
+template <bool EDGE>
+__device__ __forceinline__ void p_item(const TMaps& tm, const DomainView& D, float* smem, uint64_t* full, unsigned& it, int x0, int y0,
+                                       int z0, int z1) {
+  const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+  const int i = x0 + 4 * tx, j = y0 + ty;
+  const int m_begin = z0 - 4, m_end = z1 + 3;
+  const bool has_kc = D.kc != nullptr;
+
+  auto issue = [&](unsigned slot, int m) {
+    const int k = m - 3;
+    const bool out = k >= z0;                        // k < z1 always holds for m < m_end
+    uint64_t* bar = &full[slot];
+    float* st = smem + slot * P_STAGE_FLOATS;
+    mbar_expect_tx(bar, TILE_BYTES + (out ? P_VX_BYTES + P_VY_BYTES + TILE_BYTES + (has_kc ? TILE_BYTES : 0) : 0));
+    tma_load_3d(st + P_OFF_VZ, &tm.tile[3], bar, x0, y0, m);
+    if (out) {
+      tma_load_3d(st, &tm.vx_halo, bar, x0 - 4, y0, k);
+      tma_load_3d(st + P_OFF_VY, &tm.vy_halo, bar, x0, y0 - 4, k);
+      tma_load_3d(st + P_OFF_P, &tm.tile[0], bar, x0, y0, k);
+      if (has_kc) tma_load_3d(st + P_OFF_KC, &tm.tile[4], bar, x0, y0, k);
+    }
+  };
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < NS; ++s)
+      if (m_begin + s < m_end) issue((it + s) % NS, m_begin + s);
   }
 
   const long long rowoff = (long long)j * D.pitch + i;
-  float* __restrict__ p = D.f[0];
-  const float* __restrict__ vx = D.f[1];
-  const float* __restrict__ vz = D.f[3];
-  bool wc[4];
-#pragma unroll
-  for (int e = 0; e < 4; ++e) wc[e] = (i + e) < D.nx;
-  const bool has_l = i >= 4, has_r = (i + 4) < D.pitch;
-  const int sx = active ? slab_side(D, 0, i) : -1;
-  const int sy = active ? slab_side(D, 1, j) : -1;
-  V4 ax = zero4(), bx = zero4(), ikx = zero4();
-  float ay = 0.f, by = 0.f, iky = 1.f;
-  if (sx >= 0) {
-    ax = ldg4(D.tab[1][0][0] + i + D.ox); bx = ldg4(D.tab[1][0][1] + i + D.ox); ikx = ldg4(D.tab[1][0][2] + i + D.ox);
-  }
-  if (sy >= 0) { ay = __ldg(D.tab[1][1][0] + gj); by = __ldg(D.tab[1][1][1] + gj); iky = __ldg(D.tab[1][1][2] + gj); }
+  float* gp = D.f[0] + rowoff + (long long)z0 * D.plane;
+  const int xoff = ty * HW + 4 * tx + 4;             // own float4 inside the vx x-halo tile
+  const int yoff = ty * TX + 4 * tx;                 // row ty of the vy y-halo tile <-> y = y0-4+ty
+  const int toff = ty * TX + 4 * tx;
+  const float kc0 = D.kc0;
 
-  // vz queue: q0 = vz[k-4] ... q7 = vz[k+3]; before the first iteration q1..q7 = vz[z0-4 .. z0+2]
+  bool active = true;
+  bool wc[4] = {true, true, true, true};
+  int sx = -1, sy = -1;
+  if (EDGE) {
+    active = (i < D.nx) && (j < D.ny);
+#pragma unroll
+    for (int e = 0; e < 4; ++e) wc[e] = (i + e) < D.nx;
+    sx = active ? slab_side(D, 0, i) : -1;
+    sy = active ? slab_side(D, 1, j) : -1;
+  }
+
   V4 q0 = zero4(), q1 = zero4(), q2 = zero4(), q3 = zero4(), q4 = zero4(), q5 = zero4(), q6 = zero4(), q7 = zero4();
-  if (active) {
-    auto ldz = [&](int kk) -> V4 { return (kk >= 0 && kk < D.nz) ? ld4(vz + (long long)kk * D.plane + rowoff) : zero4(); };
-    q1 = ldz(z0 - 4); q2 = ldz(z0 - 3); q3 = ldz(z0 - 2); q4 = ldz(z0 - 1); q5 = ldz(z0); q6 = ldz(z0 + 1); q7 = ldz(z0 + 2);
-  }
 
-  int it = 0;
-  for (int k = z0; k < z1; ++k, ++it) {
-    const int s = it % PSTAGES;
-    const uint32_t parity = (it / PSTAGES) & 1;
-    const long long qk = (long long)k * D.plane + rowoff;
-    V4 vzn = zero4(), vxc = zero4(), vxl = zero4(), vxr = zero4(), p4 = zero4(), kc4 = zero4();
-    V4 psx = zero4(), psy = zero4(), psz = zero4();
-    int sz = -1;
-    if (active) {
-      if (k + 3 < D.nz) vzn = ld4(vz + qk + 3 * D.plane);
-      vxc = ld4(vx + qk);
-      if (has_l) vxl = ld4(vx + qk - 4);
-      if (has_r) vxr = ld4(vx + qk + 4);
-      p4 = ld4(p + qk);
-      if (D.kc) kc4 = ldg4(D.kc + qk);
-      else kc4 = splat4(D.kc0);
-      if (sx >= 0) psx = ld4(D.psi[1][0][sx] + psi_index(D, 0, sx, i, j, k));
-      if (sy >= 0) psy = ld4(D.psi[1][1][sy] + psi_index(D, 1, sy, i, j, k));
-      sz = slab_side(D, 2, k);
-      if (sz >= 0) psz = ld4(D.psi[1][2][sz] + psi_index(D, 2, sz, i, j, k));
-    }
-    q0 = q1; q1 = q2; q2 = q3; q3 = q4; q4 = q5; q5 = q6; q6 = q7; q7 = vzn;
+  for (int m = m_begin; m < m_end; ++m, ++it) {
+    const unsigned slot = it % NS;
+    const float* st = smem + slot * P_STAGE_FLOATS;
+    mbar_wait(&full[slot], (it / NS) & 1);
+    const int k = m - 3;
+    const bool out = k >= z0;
 
-    mbar_wait(&full[s], parity);
-    V4 dyv;
-    {
-      const float* col = tiles + s * P_STAGE_FLOATS + ty * PW + 4 * tx;     // tile row r <-> y = y0-4+r
-      const V4 r0 = ld4(col), r1 = ld4(col + PW), r2 = ld4(col + 2 * PW), r3 = ld4(col + 3 * PW);
-      const V4 r4 = ld4(col + 4 * PW), r5 = ld4(col + 5 * PW), r6 = ld4(col + 6 * PW), r7 = ld4(col + 7 * PW);
-#pragma unroll
-      for (int e = 0; e < 4; ++e)   // D-_y at node j: vy[j+l-1] = row(ty+3+l), vy[j-l] = row(ty+4-l)
-        F4(dyv, e) = stag_diff(F4(r4, e), F4(r3, e), F4(r5, e), F4(r2, e), F4(r6, e), F4(r1, e), F4(r7, e), F4(r0, e));
+    q0 = q1; q1 = q2; q2 = q3; q3 = q4; q4 = q5; q5 = q6; q6 = q7; q7 = ld4(st + P_OFF_VZ + toff);   // q7 = vz[m] = vz[k+3]
+    V4 dxv, dyv, p4, kc4;
+    if (out) {
+      const float* xr = st + xoff;
+      dxv = diff_x<false>(ld4(xr - 4), ld4(xr), ld4(xr + 4));
+      const float* col = st + P_OFF_VY + yoff;
+      // D-_y at node j: vy[j+l-1] = row(ty+3+l), vy[j-l] = row(ty+4-l)
+      dyv = diff_8(ld4(col + 4 * TX), ld4(col + 3 * TX), ld4(col + 5 * TX), ld4(col + 2 * TX), ld4(col + 6 * TX), ld4(col + TX),
+                   ld4(col + 7 * TX), ld4(col));
+      p4 = ld4(st + P_OFF_P + toff);
+      kc4 = has_kc ? ld4(st + P_OFF_KC + toff) : splat4(kc0);
     }
     __syncthreads();
-    if (threadIdx.x == 0 && k + PSTAGES < z1) {
-      mbar_expect_tx(&full[s], P_TILE_BYTES);
-      tma_load_3d(tiles + s * P_STAGE_FLOATS, &tm_vy, &full[s], x0, y0 - 4, k + PSTAGES);
-    }
-    if (!active) continue;
+    if (tid == 0 && m + NS < m_end) issue(slot, m + NS);
 
-    V4 dxv, dzv;
-    {
-      const float w[12] = {vxl.v[0], vxl.v[1], vxl.v[2], vxl.v[3], vxc.v[0], vxc.v[1], vxc.v[2], vxc.v[3], vxr.v[0], vxr.v[1], vxr.v[2], vxr.v[3]};  // vx[i-4+n]
+    if (out) {
+      // D-_z at node k: vz[k+l-1] = q(3+l), vz[k-l] = q(4-l)
+      V4 dzv = diff_8(q4, q3, q5, q2, q6, q1, q7, q0);
+      if (!EDGE) {
 #pragma unroll
-      for (int e = 0; e < 4; ++e)   // D-_x at node i+e: vx[i+e+l-1] = w(3+e+l), vx[i+e-l] = w(4+e-l)
-        F4(dxv, e) = stag_diff(w[4 + e], w[3 + e], w[5 + e], w[2 + e], w[6 + e], w[1 + e], w[7 + e], w[e]);
+        for (int e = 0; e < 4; ++e) p4.v[e] = upd(p4.v[e], kc4.v[e], __fadd_rn(__fadd_rn(dxv.v[e], dyv.v[e]), dzv.v[e]));
+        st4(gp, p4);
+      } else if (active) {
+        if (sx >= 0) {
+          float* pp = D.psi[1][0][sx] + psi_index(D, 0, sx, i, j, k);
+          V4 ps = ld4(pp);
+          const V4 a = ldg4(D.tab[1][0][0] + i + D.ox), b = ldg4(D.tab[1][0][1] + i + D.ox), ik = ldg4(D.tab[1][0][2] + i + D.ox);
 #pragma unroll
-      for (int e = 0; e < 4; ++e)   // D-_z at node k: vz[k+l-1] = q(3+l), vz[k-l] = q(4-l)
-        F4(dzv, e) = stag_diff(F4(q4, e), F4(q3, e), F4(q5, e), F4(q2, e), F4(q6, e), F4(q1, e), F4(q7, e), F4(q0, e));
+          for (int e = 0; e < 4; ++e) dxv.v[e] = cpml_apply(dxv.v[e], ps.v[e], a.v[e], b.v[e], ik.v[e]);
+          st4(pp, ps);
+        }
+        if (sy >= 0) {
+          float* pp = D.psi[1][1][sy] + psi_index(D, 1, sy, i, j, k);
+          V4 ps = ld4(pp);
+          const int gj = j + D.oy;
+          const float a = __ldg(D.tab[1][1][0] + gj), b = __ldg(D.tab[1][1][1] + gj), ik = __ldg(D.tab[1][1][2] + gj);
+#pragma unroll
+          for (int e = 0; e < 4; ++e) dyv.v[e] = cpml_apply(dyv.v[e], ps.v[e], a, b, ik);
+          st4(pp, ps);
+        }
+        const int sz = slab_side(D, 2, k);
+        if (sz >= 0) {
+          float* pp = D.psi[1][2][sz] + psi_index(D, 2, sz, i, j, k);
+          V4 ps = ld4(pp);
+          const int gk = k + D.oz;
+          const float a = __ldg(D.tab[1][2][0] + gk), b = __ldg(D.tab[1][2][1] + gk), ik = __ldg(D.tab[1][2][2] + gk);
+#pragma unroll
+          for (int e = 0; e < 4; ++e) dzv.v[e] = cpml_apply(dzv.v[e], ps.v[e], a, b, ik);
+          st4(pp, ps);
+        }
+#pragma unroll
+        for (int e = 0; e < 4; ++e)
+          p4.v[e] = wc[e] ? upd(p4.v[e], kc4.v[e], __fadd_rn(__fadd_rn(dxv.v[e], dyv.v[e]), dzv.v[e])) : 0.f;
+        st4(gp, p4);
+      }
+      gp += D.plane;
     }
-    if (sx >= 0) {
-#pragma unroll
-      for (int e = 0; e < 4; ++e) F4(dxv, e) = cpml_apply(F4(dxv, e), F4(psx, e), F4(ax, e), F4(bx, e), F4(ikx, e));
-      st4(D.psi[1][0][sx] + psi_index(D, 0, sx, i, j, k), psx);
-    }
-    if (sy >= 0) {
-#pragma unroll
-      for (int e = 0; e < 4; ++e) F4(dyv, e) = cpml_apply(F4(dyv, e), F4(psy, e), ay, by, iky);
-      st4(D.psi[1][1][sy] + psi_index(D, 1, sy, i, j, k), psy);
-    }
-    if (sz >= 0) {
-      const int gk = k + D.oz;
-      const float az = __ldg(D.tab[1][2][0] + gk), bz = __ldg(D.tab[1][2][1] + gk), ikz = __ldg(D.tab[1][2][2] + gk);
-#pragma unroll
-      for (int e = 0; e < 4; ++e) F4(dzv, e) = cpml_apply(F4(dzv, e), F4(psz, e), az, bz, ikz);
-      st4(D.psi[1][2][sz] + psi_index(D, 2, sz, i, j, k), psz);
-    }
-#pragma unroll
-    for (int e = 0; e < 4; ++e)
-      F4(p4, e) = wc[e] ? upd(F4(p4, e), F4(kc4, e), __fadd_rn(__fadd_rn(F4(dxv, e), F4(dyv, e)), F4(dzv, e))) : 0.f;
-    st4(p + qk, p4);
   }
 }
+
+__global__ void __launch_bounds__(NT, 3) update_p_tiled(const __grid_constant__ TMaps tm, const __grid_constant__ DomainView D,
+                                                        const __grid_constant__ Sched S) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  float* smem = reinterpret_cast<float*>(smem_raw);
+  __shared__ __align__(8) uint64_t full[NS];
+  __shared__ int s_item;
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int s = 0; s < NS; ++s) mbar_init(&full[s], 1);
+    fence_barrier_init();
+    if (blockIdx.x == 0) *S.other = 0u;
+  }
+  unsigned it = 0;
+  int x0, y0, z0, z1;
+  while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) {
+    if (item_is_edge(D, x0, y0, z0, z1)) p_item<true>(tm, D, smem, full, it, x0, y0, z0, z1);
+    else p_item<false>(tm, D, smem, full, it, x0, y0, z0, z1);
+  }
+}
+
 
 // ---------------------------------------------------------------- small kernels
 // p[src_s] += w_s[n] for every source, then n <- n + 1 (R14).  One block; the step counter lives on the device so
