@@ -213,6 +213,7 @@ struct fdtd_ctx {
   cudaStream_t stream;
   std::vector<Domain> doms;
   AxisTable tabs[2][3];
+  std::vector<float> dev_a[2][3];
   bool use_ref;
   int nsrc = 0, wlen = 0;
   long long* d_step;
@@ -488,7 +489,8 @@ fdtd_ctx* fdtd_create(const fdtd_params* P) {
   c->P = *P; c->G = G; c->L = L;
   c->ws = (char*)P->workspace;
   c->stream = (cudaStream_t)P->stream;
-  c->use_ref = P->kernel == FDTD_KERNEL_REF || P->boundary == FDTD_PERIODIC;
+  // the tiled kernels move whole float4s: they need Nx % 4 == 0; other grids take the reference kernels
+  c->use_ref = P->kernel == FDTD_KERNEL_REF || P->boundary == FDTD_PERIODIC || (G.gn[0] % 4) != 0;
   cudaError_t e;
   if ((e = cudaSetDevice(P->device)) != cudaSuccess) return fail(c, e, "cudaSetDevice");
   if ((e = cudaMemsetAsync(c->ws, 0, L.total, c->stream)) != cudaSuccess) return fail(c, e, "cudaMemsetAsync(workspace)");
@@ -498,7 +500,11 @@ fdtd_ctx* fdtd_create(const fdtd_params* P) {
     for (int fam = 0; fam < 2; ++fam) {
       c->tabs[fam][a] = make_axis_table(G.gn[a], P->cpml[2 * a], P->cpml[2 * a + 1], fam == 0, *P);
       const AxisTable& t = c->tabs[fam][a];
-      const float* src[3] = {t.a.data(), t.b.data(), t.ik.data()};
+      // device copy of the half-node `a`: 0 at the pinned last half node (R3), so its psi stays 0 as in the
+      // recurrence, which never updates that node; fdtd_cpml_table returns the plain formula values
+      c->dev_a[fam][a] = t.a;
+      if (fam == 0 && P->boundary == FDTD_WALL) c->dev_a[fam][a][G.gn[a] - 1] = 0.0f;
+      const float* src[3] = {c->dev_a[fam][a].data(), t.b.data(), t.ik.data()};
       for (int k = 0; k < 3; ++k)
         if ((e = cudaMemcpyAsync(c->ws + L.tab[fam][a][k], src[k], (size_t)L.tablen[a] * 4, cudaMemcpyHostToDevice, c->stream)) != cudaSuccess)
           return fail(c, e, "cudaMemcpyAsync(tables)");

@@ -166,13 +166,16 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 
 // ---------------------------------------------------------------- tiled kernels
 // Persistent CTAs (grid = resident CTAs of the whole GPU) pull work items from an atomic counter.  One item is a
-// 64x16 (x,y) tile over a chunk of z planes.  Every operand of an item arrives in shared memory through TMA into a
-// 3-stage ring (one mbarrier per stage, armed with the stage's byte count), so the streaming loads run ahead of the
-// arithmetic without holding registers; results leave through 128-bit stores.  z neighbours live in a register queue.
-// Items away from every boundary and CPML slab take a mask-free path; the others take the general path.
+// 64x16 (x,y) tile over a chunk of z planes.  Every streamed operand of an item arrives in shared memory through TMA
+// into an NS-stage ring: a "full" mbarrier per stage is armed with the stage's byte count, an "empty" mbarrier
+// collects one arrival per warp once the warp has read the stage, and one elected thread refills the stage used in
+// the previous iteration — no CTA-wide barrier inside the plane loop.  Results leave through 128-bit stores; the
+// z neighbours live in a register queue.  CPML slabs are handled by block-uniform branches (x / y per item, z per
+// plane) with slab-local psi arrays read and written directly.
 constexpr int TX = 64;             // tile width in x (floats): 16 lanes x 4
 constexpr int TY = 16;             // tile height in y (rows)
 constexpr int NT = 256;            // threads per CTA
+constexpr int NW = NT / 32;        // warps per CTA
 constexpr int NS = 3;              // ring stages
 constexpr int HW = TX + 8;         // x-halo tile width: columns x0-4 .. x0+TX+3
 constexpr int VH = TY + 7;         // p rows for update_v: y0-3 .. y0+TY+3
@@ -216,7 +219,6 @@ __device__ __forceinline__ V4 ld4(const float* p) { return from4(*reinterpret_ca
 __device__ __forceinline__ void st4(float* p, const V4& a) { *reinterpret_cast<float4*>(p) = make_float4(a.v[0], a.v[1], a.v[2], a.v[3]); }
 __device__ __forceinline__ V4 splat4(float x) { V4 r; r.v[0] = r.v[1] = r.v[2] = r.v[3] = x; return r; }
 __device__ __forceinline__ V4 zero4() { return splat4(0.f); }
-#define F4(a, e) ((a).v[e])
 
 // D along x for four consecutive outputs from the 12 values w[n] = f[i-4+n]:
 //   FWD (D+ at i+e+1/2): f[i+e+l] - f[i+e-l+1];  BWD (D- at node i+e): f[i+e+l-1] - f[i+e-l]
@@ -226,7 +228,7 @@ __device__ __forceinline__ V4 diff_x(const V4& l, const V4& c, const V4& r) {
   V4 d;
 #pragma unroll
   for (int e = 0; e < 4; ++e) {
-    const int o = FWD ? 4 + e : 3 + e;   // index of the first "hi" operand minus 1
+    const int o = FWD ? 4 + e : 3 + e;
     d.v[e] = stag_diff(w[o + 1], w[o], w[o + 2], w[o - 1], w[o + 3], w[o - 2], w[o + 4], w[o - 3]);
   }
   return d;
@@ -238,12 +240,39 @@ __device__ __forceinline__ V4 diff_8(const V4& h1, const V4& l1, const V4& h2, c
   for (int e = 0; e < 4; ++e) d.v[e] = stag_diff(h1.v[e], l1.v[e], h2.v[e], l2.v[e], h3.v[e], l3.v[e], h4.v[e], l4.v[e]);
   return d;
 }
+__device__ __forceinline__ void cpml4(V4& d, V4& ps, const V4& a, const V4& b, const V4& ik) {
+#pragma unroll
+  for (int e = 0; e < 4; ++e) d.v[e] = cpml_apply(d.v[e], ps.v[e], a.v[e], b.v[e], ik.v[e]);
+}
+__device__ __forceinline__ void cpml4s(V4& d, V4& ps, float a, float b, float ik) {
+#pragma unroll
+  for (int e = 0; e < 4; ++e) d.v[e] = cpml_apply(d.v[e], ps.v[e], a, b, ik);
+}
+
+// ring bookkeeping shared by both kernels
+struct Ring {
+  uint64_t* full;
+  uint64_t* empty;
+};
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+// the warp has finished reading stage `slot`
+__device__ __forceinline__ void release_stage(const Ring& R, unsigned slot) {
+  __syncwarp();
+  if ((threadIdx.x & 31) == 0) mbar_arrive(&R.empty[slot]);
+}
+
+__device__ __forceinline__ bool touches(const DomainView& D, int axis, int lo, int hi) {
+  return (D.ln[axis][0] > 0 && lo < D.ls[axis][0] + D.ln[axis][0] && hi > D.ls[axis][0]) ||
+         (D.ln[axis][1] > 0 && lo < D.ls[axis][1] + D.ln[axis][1] && hi > D.ls[axis][1]);
+}
 
 // ---- velocity sub-update: v_a <- v_a - B [(1/kappa_a) D+_a p + psi_va] for one item.
 // On arrival of stage "p plane m": vx, vy of plane m are updated from the tile, p[m] enters the register queue and
-// vz of plane m-4 is updated from the queue (D+_z at k+1/2 reads p[k-3 .. k+4]).
-template <bool EDGE>
-__device__ __forceinline__ void v_item(const TMaps& tm, const DomainView& D, float* smem, uint64_t* full, unsigned& it, int x0, int y0,
+// vz of plane m-4 is updated from the queue (D+_z at k+1/2 reads p[k-3 .. k+4]).  The pinned last half node of each
+// axis (R3) is kept by a zero update coefficient (its psi stays 0 through a zero `a` in the device table).
+__device__ __forceinline__ void v_item(const TMaps& tm, const DomainView& D, float* smem, const Ring& R, unsigned& it, int x0, int y0,
                                        int z0, int z1) {
   const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
   const int i = x0 + 4 * tx, j = y0 + ty;
@@ -251,7 +280,7 @@ __device__ __forceinline__ void v_item(const TMaps& tm, const DomainView& D, flo
 
   auto issue = [&](unsigned slot, int m) {
     const bool xy = m >= z0 && m < z1, zz = (m - 4) >= z0 && (m - 4) < z1;
-    uint64_t* bar = &full[slot];
+    uint64_t* bar = &R.full[slot];
     float* st = smem + slot * V_STAGE_FLOATS;
     mbar_expect_tx(bar, V_P_BYTES + (xy ? 2 * TILE_BYTES : 0) + (zz ? TILE_BYTES : 0));
     tma_load_3d(st, &tm.p_halo, bar, x0 - 4, y0 - 3, m);
@@ -267,6 +296,7 @@ __device__ __forceinline__ void v_item(const TMaps& tm, const DomainView& D, flo
       if (m_begin + s < m_end) issue((it + s) % NS, m_begin + s);
   }
 
+  const bool active = (i < D.nx) && (j < D.ny);
   const float B = D.b0;
   const long long rowoff = (long long)j * D.pitch + i;
   float* gvx = D.f[1] + rowoff + (long long)z0 * D.plane;
@@ -274,32 +304,40 @@ __device__ __forceinline__ void v_item(const TMaps& tm, const DomainView& D, flo
   float* gvz = D.f[3] + rowoff + (long long)z0 * D.plane;
   const int poff = (ty + 3) * HW + 4 * tx + 4;      // own float4 inside the p halo tile
   const int toff = ty * TX + 4 * tx;                // own float4 inside a plain tile
-
-  // general path only: masks and CPML bookkeeping
-  bool active = true, wy_row = true;
-  bool wc[4] = {true, true, true, true}, wx[4] = {true, true, true, true};
-  int sx = -1, sy = -1;
-  if (EDGE) {
-    active = (i < D.nx) && (j < D.ny);
-#pragma unroll
-    for (int e = 0; e < 4; ++e) {
-      wc[e] = (i + e) < D.nx;                                         // real column (padding columns stay 0)
-      wx[e] = wc[e] && (i + e + D.ox) != D.gn[0] - 1;                 // not the pinned last half node (R3)
-    }
-    wy_row = (j + D.oy) != D.gn[1] - 1;
-    sx = active ? slab_side(D, 0, i) : -1;
-    sy = active ? slab_side(D, 1, j) : -1;
-  }
+  // pinned last half nodes: zero coefficient
+  const float Bx3 = (i + 3 + D.ox) == D.gn[0] - 1 ? 0.f : B;
+  const float By = (j + D.oy) == D.gn[1] - 1 ? 0.f : B;
+  // CPML: block-uniform "does this item touch an x / y slab", per-thread "is my float4 / row inside one"
+  const bool any_x = touches(D, 0, x0, x0 + TX), any_y = touches(D, 1, y0, y0 + TY);
+  const int sx = (any_x && active) ? slab_side(D, 0, i) : -1;
+  const int sy = (any_y && active) ? slab_side(D, 1, j) : -1;
+  float* ppx = sx >= 0 ? D.psi[0][0][sx] + psi_index(D, 0, sx, i, j, z0) : nullptr;
+  float* ppy = sy >= 0 ? D.psi[0][1][sy] + psi_index(D, 1, sy, i, j, z0) : nullptr;
+  const long long stride_px = sx >= 0 ? (long long)D.ny * D.ln[0][sx] : 0;
+  const long long stride_py = sy >= 0 ? (long long)D.ln[1][sy] * D.pitch : 0;
 
   V4 q0 = zero4(), q1 = zero4(), q2 = zero4(), q3 = zero4(), q4 = zero4(), q5 = zero4(), q6 = zero4(), q7 = zero4();
 
   for (int m = m_begin; m < m_end; ++m, ++it) {
     const unsigned slot = it % NS;
-    const float* st = smem + slot * V_STAGE_FLOATS;
-    mbar_wait(&full[slot], (it / NS) & 1);
     const bool xy = m >= z0 && m < z1;
     const int kz = m - 4;
     const bool zz = kz >= z0 && kz < z1;
+    // psi of this iteration: issue the loads before waiting on the tile
+    V4 psx, psy, psz;
+    const int sz = zz ? slab_side(D, 2, kz) : -1;
+    float* ppz = nullptr;
+    if (xy && sx >= 0) psx = ld4(ppx);
+    if (xy && sy >= 0) psy = ld4(ppy);
+    if (sz >= 0 && active) { ppz = D.psi[0][2][sz] + psi_index(D, 2, sz, i, j, kz); psz = ld4(ppz); }
+    // producer duty: refill the stage every warp released in the previous iteration
+    if (tid == 0 && m > m_begin && (m - 1 + NS) < m_end) {
+      const unsigned ps = (it - 1) % NS;
+      mbar_wait(&R.empty[ps], ((it - 1) / NS) & 1);
+      issue(ps, m - 1 + NS);
+    }
+    const float* st = smem + slot * V_STAGE_FLOATS;
+    mbar_wait(&R.full[slot], (it / NS) & 1);
 
     const float* row = st + poff;
     const V4 c = ld4(row);
@@ -312,91 +350,53 @@ __device__ __forceinline__ void v_item(const TMaps& tm, const DomainView& D, flo
       vy4 = ld4(st + V_OFF_VY + toff);
     }
     if (zz) vz4 = ld4(st + V_OFF_VZ + toff);
+    release_stage(R, slot);
     q0 = q1; q1 = q2; q2 = q3; q3 = q4; q4 = q5; q5 = q6; q6 = q7; q7 = c;     // q7 = p[m] ... q0 = p[m-7]
-    __syncthreads();                                                             // every thread is done with this stage
-    if (tid == 0 && m + NS < m_end) issue(slot, m + NS);
 
     if (xy) {
-      if (!EDGE) {
-#pragma unroll
-        for (int e = 0; e < 4; ++e) { vx4.v[e] = upd(vx4.v[e], B, dxv.v[e]); vy4.v[e] = upd(vy4.v[e], B, dyv.v[e]); }
-        st4(gvx, vx4);
-        st4(gvy, vy4);
-      } else if (active) {
+      if (any_x) {
         if (sx >= 0) {
-          float* pp = D.psi[0][0][sx] + psi_index(D, 0, sx, i, j, m);
-          V4 ps = ld4(pp);
-          const V4 a = ldg4(D.tab[0][0][0] + i + D.ox), b = ldg4(D.tab[0][0][1] + i + D.ox), ik = ldg4(D.tab[0][0][2] + i + D.ox);
-#pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            const float old = ps.v[e];
-            dxv.v[e] = cpml_apply(dxv.v[e], ps.v[e], a.v[e], b.v[e], ik.v[e]);
-            if (!wx[e]) ps.v[e] = old;                                 // the pinned half node keeps its psi too
-          }
-          st4(pp, ps);
+          const int gi = i + D.ox;
+          cpml4(dxv, psx, ldg4(D.tab[0][0][0] + gi), ldg4(D.tab[0][0][1] + gi), ldg4(D.tab[0][0][2] + gi));
+          st4(ppx, psx);
+          ppx += stride_px;
         }
-        if (sy >= 0 && wy_row) {
-          float* pp = D.psi[0][1][sy] + psi_index(D, 1, sy, i, j, m);
-          V4 ps = ld4(pp);
-          const int gj = j + D.oy;
-          const float a = __ldg(D.tab[0][1][0] + gj), b = __ldg(D.tab[0][1][1] + gj), ik = __ldg(D.tab[0][1][2] + gj);
-#pragma unroll
-          for (int e = 0; e < 4; ++e) dyv.v[e] = cpml_apply(dyv.v[e], ps.v[e], a, b, ik);
-          st4(pp, ps);
-        }
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-          const float nvx = upd(vx4.v[e], B, dxv.v[e]), nvy = upd(vy4.v[e], B, dyv.v[e]);
-          vx4.v[e] = wx[e] ? nvx : (wc[e] ? vx4.v[e] : 0.f);
-          vy4.v[e] = wc[e] ? (wy_row ? nvy : vy4.v[e]) : 0.f;
-        }
-        st4(gvx, vx4);
-        st4(gvy, vy4);
       }
+      if (any_y) {
+        if (sy >= 0) {
+          const int gj = j + D.oy;
+          cpml4s(dyv, psy, __ldg(D.tab[0][1][0] + gj), __ldg(D.tab[0][1][1] + gj), __ldg(D.tab[0][1][2] + gj));
+          st4(ppy, psy);
+          ppy += stride_py;
+        }
+      }
+      vx4.v[0] = upd(vx4.v[0], B, dxv.v[0]); vx4.v[1] = upd(vx4.v[1], B, dxv.v[1]);
+      vx4.v[2] = upd(vx4.v[2], B, dxv.v[2]); vx4.v[3] = upd(vx4.v[3], Bx3, dxv.v[3]);
+#pragma unroll
+      for (int e = 0; e < 4; ++e) vy4.v[e] = upd(vy4.v[e], By, dyv.v[e]);
+      if (active) { st4(gvx, vx4); st4(gvy, vy4); }
       gvx += D.plane;
       gvy += D.plane;
     }
     if (zz) {
       // D+_z at kz+1/2: p[kz+l] = q(3+l), p[kz-l+1] = q(4-l)
       V4 dzv = diff_8(q4, q3, q5, q2, q6, q1, q7, q0);
-      if (!EDGE) {
-#pragma unroll
-        for (int e = 0; e < 4; ++e) vz4.v[e] = upd(vz4.v[e], B, dzv.v[e]);
-        st4(gvz, vz4);
-      } else if (active && (kz + D.oz) != D.gn[2] - 1) {
-        const int sz = slab_side(D, 2, kz);
-        if (sz >= 0) {
-          float* pp = D.psi[0][2][sz] + psi_index(D, 2, sz, i, j, kz);
-          V4 ps = ld4(pp);
-          const int gk = kz + D.oz;
-          const float a = __ldg(D.tab[0][2][0] + gk), b = __ldg(D.tab[0][2][1] + gk), ik = __ldg(D.tab[0][2][2] + gk);
-#pragma unroll
-          for (int e = 0; e < 4; ++e) dzv.v[e] = cpml_apply(dzv.v[e], ps.v[e], a, b, ik);
-          st4(pp, ps);
-        }
-#pragma unroll
-        for (int e = 0; e < 4; ++e) vz4.v[e] = wc[e] ? upd(vz4.v[e], B, dzv.v[e]) : 0.f;
-        st4(gvz, vz4);
+      const int gk = kz + D.oz;
+      if (sz >= 0 && active) {
+        cpml4s(dzv, psz, __ldg(D.tab[0][2][0] + gk), __ldg(D.tab[0][2][1] + gk), __ldg(D.tab[0][2][2] + gk));
+        st4(ppz, psz);
       }
+      const float Bz = gk == D.gn[2] - 1 ? 0.f : B;
+#pragma unroll
+      for (int e = 0; e < 4; ++e) vz4.v[e] = upd(vz4.v[e], Bz, dzv.v[e]);
+      if (active) st4(gvz, vz4);
       gvz += D.plane;
     }
   }
 }
 
-// does the item [x0,x0+TX) x [y0,y0+TY) x [z0,z1) need masks or CPML code?
-__device__ __forceinline__ bool item_is_edge(const DomainView& D, int x0, int y0, int z0, int z1) {
-  if (x0 + TX >= D.nx || y0 + TY >= D.ny || z1 >= D.nz) return true;     // ragged tile or the pinned last index
-  const int lo[3] = {x0, y0, z0}, hi[3] = {x0 + TX, y0 + TY, z1};
-#pragma unroll
-  for (int a = 0; a < 3; ++a)
-#pragma unroll
-    for (int s = 0; s < 2; ++s)
-      if (D.ln[a][s] > 0 && lo[a] < D.ls[a][s] + D.ln[a][s] && hi[a] > D.ls[a][s]) return true;
-  return false;
-}
-
 __device__ __forceinline__ bool next_item(const Sched& S, int* s_item, int& x0, int& y0, int& z0, int& z1, int nz) {
-  __syncthreads();                                   // previous item fully consumed (smem tiles and s_item)
+  __syncthreads();                                   // previous item fully consumed (all stages released, s_item read)
   if (threadIdx.x == 0) *s_item = (int)atomicAdd(S.counter, 1u);
   __syncthreads();
   const int item = *s_item;
@@ -407,31 +407,33 @@ __device__ __forceinline__ bool next_item(const Sched& S, int* s_item, int& x0, 
   return true;
 }
 
+__device__ __forceinline__ void ring_init(uint64_t* full, uint64_t* empty, unsigned int* other) {
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int s = 0; s < NS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NW); }
+    fence_barrier_init();
+    if (blockIdx.x == 0) *other = 0u;                // arm the next launch's work counter
+  }
+}
+
 __global__ void __launch_bounds__(NT, 3) update_v_tiled(const __grid_constant__ TMaps tm, const __grid_constant__ DomainView D,
                                                         const __grid_constant__ Sched S) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   float* smem = reinterpret_cast<float*>(smem_raw);
   __shared__ __align__(8) uint64_t full[NS];
+  __shared__ __align__(8) uint64_t empty[NS];
   __shared__ int s_item;
-  if (threadIdx.x == 0) {
-#pragma unroll
-    for (int s = 0; s < NS; ++s) mbar_init(&full[s], 1);
-    fence_barrier_init();
-    if (blockIdx.x == 0) *S.other = 0u;              // arm the next launch's work counter
-  }
+  ring_init(full, empty, S.other);
+  const Ring R{full, empty};
   unsigned it = 0;
   int x0, y0, z0, z1;
-  while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) {
-    if (item_is_edge(D, x0, y0, z0, z1)) v_item<true>(tm, D, smem, full, it, x0, y0, z0, z1);
-    else v_item<false>(tm, D, smem, full, it, x0, y0, z0, z1);
-  }
+  while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) v_item(tm, D, smem, R, it, x0, y0, z0, z1);
 }
 
 // ---- pressure sub-update: p <- p - Kc [sum_a (1/kappa_a) D-_a v_a + psi_pa] for one item.
 // Stage "vz plane m" also carries vx (x-halo tile), vy (y-halo tile), p and Kc of plane k = m-3; vz[m] enters the
 // register queue and p[k] is updated (D-_z at node k reads vz[k-4 .. k+3]).
-template <bool EDGE>
-__device__ __forceinline__ void p_item(const TMaps& tm, const DomainView& D, float* smem, uint64_t* full, unsigned& it, int x0, int y0,
+__device__ __forceinline__ void p_item(const TMaps& tm, const DomainView& D, float* smem, const Ring& R, unsigned& it, int x0, int y0,
                                        int z0, int z1) {
   const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
   const int i = x0 + 4 * tx, j = y0 + ty;
@@ -441,7 +443,7 @@ __device__ __forceinline__ void p_item(const TMaps& tm, const DomainView& D, flo
   auto issue = [&](unsigned slot, int m) {
     const int k = m - 3;
     const bool out = k >= z0;                        // k < z1 always holds for m < m_end
-    uint64_t* bar = &full[slot];
+    uint64_t* bar = &R.full[slot];
     float* st = smem + slot * P_STAGE_FLOATS;
     mbar_expect_tx(bar, TILE_BYTES + (out ? P_VX_BYTES + P_VY_BYTES + TILE_BYTES + (has_kc ? TILE_BYTES : 0) : 0));
     tma_load_3d(st + P_OFF_VZ, &tm.tile[3], bar, x0, y0, m);
@@ -458,88 +460,81 @@ __device__ __forceinline__ void p_item(const TMaps& tm, const DomainView& D, flo
       if (m_begin + s < m_end) issue((it + s) % NS, m_begin + s);
   }
 
+  const bool active = (i < D.nx) && (j < D.ny);
   const long long rowoff = (long long)j * D.pitch + i;
   float* gp = D.f[0] + rowoff + (long long)z0 * D.plane;
   const int xoff = ty * HW + 4 * tx + 4;             // own float4 inside the vx x-halo tile
-  const int yoff = ty * TX + 4 * tx;                 // row ty of the vy y-halo tile <-> y = y0-4+ty
-  const int toff = ty * TX + 4 * tx;
+  const int toff = ty * TX + 4 * tx;                 // own float4 in a plain tile; row ty of the vy tile <-> y = y0-4+ty
   const float kc0 = D.kc0;
-
-  bool active = true;
-  bool wc[4] = {true, true, true, true};
-  int sx = -1, sy = -1;
-  if (EDGE) {
-    active = (i < D.nx) && (j < D.ny);
-#pragma unroll
-    for (int e = 0; e < 4; ++e) wc[e] = (i + e) < D.nx;
-    sx = active ? slab_side(D, 0, i) : -1;
-    sy = active ? slab_side(D, 1, j) : -1;
-  }
+  const bool any_x = touches(D, 0, x0, x0 + TX), any_y = touches(D, 1, y0, y0 + TY);
+  const int sx = (any_x && active) ? slab_side(D, 0, i) : -1;
+  const int sy = (any_y && active) ? slab_side(D, 1, j) : -1;
+  float* ppx = sx >= 0 ? D.psi[1][0][sx] + psi_index(D, 0, sx, i, j, z0) : nullptr;
+  float* ppy = sy >= 0 ? D.psi[1][1][sy] + psi_index(D, 1, sy, i, j, z0) : nullptr;
+  const long long stride_px = sx >= 0 ? (long long)D.ny * D.ln[0][sx] : 0;
+  const long long stride_py = sy >= 0 ? (long long)D.ln[1][sy] * D.pitch : 0;
 
   V4 q0 = zero4(), q1 = zero4(), q2 = zero4(), q3 = zero4(), q4 = zero4(), q5 = zero4(), q6 = zero4(), q7 = zero4();
 
   for (int m = m_begin; m < m_end; ++m, ++it) {
     const unsigned slot = it % NS;
-    const float* st = smem + slot * P_STAGE_FLOATS;
-    mbar_wait(&full[slot], (it / NS) & 1);
     const int k = m - 3;
     const bool out = k >= z0;
+    V4 psx, psy, psz;
+    const int sz = out ? slab_side(D, 2, k) : -1;
+    float* ppz = nullptr;
+    if (out && sx >= 0) psx = ld4(ppx);
+    if (out && sy >= 0) psy = ld4(ppy);
+    if (sz >= 0 && active) { ppz = D.psi[1][2][sz] + psi_index(D, 2, sz, i, j, k); psz = ld4(ppz); }
+    if (tid == 0 && m > m_begin && (m - 1 + NS) < m_end) {
+      const unsigned ps = (it - 1) % NS;
+      mbar_wait(&R.empty[ps], ((it - 1) / NS) & 1);
+      issue(ps, m - 1 + NS);
+    }
+    const float* st = smem + slot * P_STAGE_FLOATS;
+    mbar_wait(&R.full[slot], (it / NS) & 1);
 
     q0 = q1; q1 = q2; q2 = q3; q3 = q4; q4 = q5; q5 = q6; q6 = q7; q7 = ld4(st + P_OFF_VZ + toff);   // q7 = vz[m] = vz[k+3]
     V4 dxv, dyv, p4, kc4;
     if (out) {
       const float* xr = st + xoff;
       dxv = diff_x<false>(ld4(xr - 4), ld4(xr), ld4(xr + 4));
-      const float* col = st + P_OFF_VY + yoff;
+      const float* col = st + P_OFF_VY + toff;
       // D-_y at node j: vy[j+l-1] = row(ty+3+l), vy[j-l] = row(ty+4-l)
       dyv = diff_8(ld4(col + 4 * TX), ld4(col + 3 * TX), ld4(col + 5 * TX), ld4(col + 2 * TX), ld4(col + 6 * TX), ld4(col + TX),
                    ld4(col + 7 * TX), ld4(col));
       p4 = ld4(st + P_OFF_P + toff);
       kc4 = has_kc ? ld4(st + P_OFF_KC + toff) : splat4(kc0);
     }
-    __syncthreads();
-    if (tid == 0 && m + NS < m_end) issue(slot, m + NS);
+    release_stage(R, slot);
 
     if (out) {
       // D-_z at node k: vz[k+l-1] = q(3+l), vz[k-l] = q(4-l)
       V4 dzv = diff_8(q4, q3, q5, q2, q6, q1, q7, q0);
-      if (!EDGE) {
-#pragma unroll
-        for (int e = 0; e < 4; ++e) p4.v[e] = upd(p4.v[e], kc4.v[e], __fadd_rn(__fadd_rn(dxv.v[e], dyv.v[e]), dzv.v[e]));
-        st4(gp, p4);
-      } else if (active) {
+      if (any_x) {
         if (sx >= 0) {
-          float* pp = D.psi[1][0][sx] + psi_index(D, 0, sx, i, j, k);
-          V4 ps = ld4(pp);
-          const V4 a = ldg4(D.tab[1][0][0] + i + D.ox), b = ldg4(D.tab[1][0][1] + i + D.ox), ik = ldg4(D.tab[1][0][2] + i + D.ox);
-#pragma unroll
-          for (int e = 0; e < 4; ++e) dxv.v[e] = cpml_apply(dxv.v[e], ps.v[e], a.v[e], b.v[e], ik.v[e]);
-          st4(pp, ps);
+          const int gi = i + D.ox;
+          cpml4(dxv, psx, ldg4(D.tab[1][0][0] + gi), ldg4(D.tab[1][0][1] + gi), ldg4(D.tab[1][0][2] + gi));
+          st4(ppx, psx);
+          ppx += stride_px;
         }
-        if (sy >= 0) {
-          float* pp = D.psi[1][1][sy] + psi_index(D, 1, sy, i, j, k);
-          V4 ps = ld4(pp);
-          const int gj = j + D.oy;
-          const float a = __ldg(D.tab[1][1][0] + gj), b = __ldg(D.tab[1][1][1] + gj), ik = __ldg(D.tab[1][1][2] + gj);
-#pragma unroll
-          for (int e = 0; e < 4; ++e) dyv.v[e] = cpml_apply(dyv.v[e], ps.v[e], a, b, ik);
-          st4(pp, ps);
-        }
-        const int sz = slab_side(D, 2, k);
-        if (sz >= 0) {
-          float* pp = D.psi[1][2][sz] + psi_index(D, 2, sz, i, j, k);
-          V4 ps = ld4(pp);
-          const int gk = k + D.oz;
-          const float a = __ldg(D.tab[1][2][0] + gk), b = __ldg(D.tab[1][2][1] + gk), ik = __ldg(D.tab[1][2][2] + gk);
-#pragma unroll
-          for (int e = 0; e < 4; ++e) dzv.v[e] = cpml_apply(dzv.v[e], ps.v[e], a, b, ik);
-          st4(pp, ps);
-        }
-#pragma unroll
-        for (int e = 0; e < 4; ++e)
-          p4.v[e] = wc[e] ? upd(p4.v[e], kc4.v[e], __fadd_rn(__fadd_rn(dxv.v[e], dyv.v[e]), dzv.v[e])) : 0.f;
-        st4(gp, p4);
       }
+      if (any_y) {
+        if (sy >= 0) {
+          const int gj = j + D.oy;
+          cpml4s(dyv, psy, __ldg(D.tab[1][1][0] + gj), __ldg(D.tab[1][1][1] + gj), __ldg(D.tab[1][1][2] + gj));
+          st4(ppy, psy);
+          ppy += stride_py;
+        }
+      }
+      if (sz >= 0 && active) {
+        const int gk = k + D.oz;
+        cpml4s(dzv, psz, __ldg(D.tab[1][2][0] + gk), __ldg(D.tab[1][2][1] + gk), __ldg(D.tab[1][2][2] + gk));
+        st4(ppz, psz);
+      }
+#pragma unroll
+      for (int e = 0; e < 4; ++e) p4.v[e] = upd(p4.v[e], kc4.v[e], __fadd_rn(__fadd_rn(dxv.v[e], dyv.v[e]), dzv.v[e]));
+      if (active) st4(gp, p4);
       gp += D.plane;
     }
   }
@@ -550,19 +545,13 @@ __global__ void __launch_bounds__(NT, 3) update_p_tiled(const __grid_constant__ 
   extern __shared__ __align__(128) unsigned char smem_raw[];
   float* smem = reinterpret_cast<float*>(smem_raw);
   __shared__ __align__(8) uint64_t full[NS];
+  __shared__ __align__(8) uint64_t empty[NS];
   __shared__ int s_item;
-  if (threadIdx.x == 0) {
-#pragma unroll
-    for (int s = 0; s < NS; ++s) mbar_init(&full[s], 1);
-    fence_barrier_init();
-    if (blockIdx.x == 0) *S.other = 0u;
-  }
+  ring_init(full, empty, S.other);
+  const Ring R{full, empty};
   unsigned it = 0;
   int x0, y0, z0, z1;
-  while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) {
-    if (item_is_edge(D, x0, y0, z0, z1)) p_item<true>(tm, D, smem, full, it, x0, y0, z0, z1);
-    else p_item<false>(tm, D, smem, full, it, x0, y0, z0, z1);
-  }
+  while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) p_item(tm, D, smem, R, it, x0, y0, z0, z1);
 }
 
 
