@@ -176,7 +176,7 @@ constexpr int TX = 64;             // tile width in x (floats): 16 lanes x 4
 constexpr int TY = 16;             // tile height in y (rows)
 constexpr int NT = 256;            // threads per CTA
 constexpr int NW = NT / 32;        // warps per CTA
-constexpr int NS = 3;              // ring stages
+constexpr int NS = 4;              // ring stages
 constexpr int HW = TX + 8;         // x-halo tile width: columns x0-4 .. x0+TX+3
 constexpr int VH = TY + 7;         // p rows for update_v: y0-3 .. y0+TY+3
 constexpr int PH = TY + 8;         // vy rows for update_p: y0-4 .. y0+TY+3
@@ -416,7 +416,7 @@ __device__ __forceinline__ void ring_init(uint64_t* full, uint64_t* empty, unsig
   }
 }
 
-__global__ void __launch_bounds__(NT, 3) update_v_tiled(const __grid_constant__ TMaps tm, const __grid_constant__ DomainView D,
+__global__ void __launch_bounds__(NT, 2) update_v_tiled(const __grid_constant__ TMaps tm, const __grid_constant__ DomainView D,
                                                         const __grid_constant__ Sched S) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   float* smem = reinterpret_cast<float*>(smem_raw);
@@ -540,7 +540,7 @@ __device__ __forceinline__ void p_item(const TMaps& tm, const DomainView& D, flo
   }
 }
 
-__global__ void __launch_bounds__(NT, 3) update_p_tiled(const __grid_constant__ TMaps tm, const __grid_constant__ DomainView D,
+__global__ void __launch_bounds__(NT, 2) update_p_tiled(const __grid_constant__ TMaps tm, const __grid_constant__ DomainView D,
                                                         const __grid_constant__ Sched S) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   float* smem = reinterpret_cast<float*>(smem_raw);
