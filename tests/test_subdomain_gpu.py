@@ -1,0 +1,82 @@
+"""BASELINE config 5: the single-GPU pencil-yz subdomain mode (1x2x2 in-HBM subdomains, ghost width g, m sub-updates
+between halo exchanges) must reproduce the monolithic run bit for bit (Table 9, P:274-288,
+made exact; readings R20, R21, R24)."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2606_06910_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2606_06910_b200 import binding
+    return binding
+
+
+def _run(B, shape, cpml, steps, random_state, src, **kw):
+    base = dict(dt=0.4, cpml_alpha_max=math.pi * inputs.F0)
+    sim = B.Fdtd(shape, cpml, **base, **kw)
+    if random_state:
+        for f in range(4):
+            sim.fill_hash(f, 17, 0.5)
+    sim.set_sources(src, np.tile(inputs.ricker(steps, 0.4, t0=4.0), (len(src), 1)))
+    sim.step(steps)
+    out = [sim.get_field(f) for f in range(4)] + [sim.get_psi(q) for q in range(6)]
+    launches = sim.launch_count()
+    sim.destroy()
+    return out, launches
+
+
+def _same_bits(a, b):
+    return np.array_equal(a.view(np.uint32), b.view(np.uint32))
+
+
+@pytest.mark.parametrize("kernel", [0, 1])
+@pytest.mark.parametrize("g,m", [(4, 1), (8, 2), (16, 4), (12, 2), (32, 8)])
+def test_subdomains_bit_identical_small(B, kernel, g, m):
+    shape, cpml = (72, 80, 88), (8, 8, 8, 8, 8, 8)            # total 88 x 96 x 104: subdomains 88 x 48 x 52 (+ ghosts)
+    src = [(44, 48, 52), (5, 47, 51), (80, 60, 20)]           # on the 4-subdomain corner, inside a layer, off-centre
+    ref, _ = _run(B, shape, cpml, 24, True, src, kernel=kernel)
+    sub, launches = _run(B, shape, cpml, 24, True, src, kernel=kernel, decomp=(1, 2, 2), ghost=g, substeps=m)
+    names = ["p", "vx", "vy", "vz", "psi_vx", "psi_vy", "psi_vz", "psi_px", "psi_py", "psi_pz"]
+    for n, a, b in zip(names, ref, sub):
+        assert _same_bits(a, b), (n, float(np.abs(a - b).max()))
+    assert launches > 24 * 2 * 4                                # 4 subdomains x 2 sub-updates per step + exchanges
+
+
+def test_insufficient_ghost_is_rejected(B):
+    with pytest.raises(B.FdtdError):
+        B.Fdtd((64,) * 3, (8,) * 6, dt=0.4, decomp=(1, 2, 2), ghost=8, substeps=3)
+
+
+def test_other_layouts_slab_and_more_subdomains(B):
+    """1x1x4 (slab-z) and 1x4x2 also reproduce the monolithic run."""
+    shape, cpml = (40, 64, 96), (4, 4, 8, 8, 16, 16)
+    src = [(24, 40, 64)]
+    ref, _ = _run(B, shape, cpml, 12, True, src)
+    for decomp in ((1, 1, 4), (1, 4, 2)):
+        sub, _ = _run(B, shape, cpml, 12, True, src, decomp=decomp, ghost=8, substeps=2)
+        for a, b in zip(ref, sub):
+            assert _same_bits(a, b), decomp
+
+
+def test_config5_full_size_bit_identical(B):
+    """The full BASELINE config 5: 512^3 + 20-cell CPML as 1x2x2, centre source on the 4-subdomain corner, 400 steps,
+    (g, m) = (8, 2) — the paper's s = 1 — compared with the monolithic kernel on all four fields."""
+    w = inputs.config(5)
+    mono = B.from_workload(w, decomp=(1, 1, 1), ghost=0, substeps=0)
+    mono.step(w.steps)
+    sub = B.from_workload(w, decomp=(1, 2, 2), ghost=8, substeps=2)
+    sub.step(w.steps)
+    for f in range(4):
+        a, b = mono.get_field(f), sub.get_field(f)
+        assert np.abs(a).max() > 0
+        assert _same_bits(a, b), f
+    mono.destroy()
+    sub.destroy()
