@@ -86,6 +86,23 @@ def ncu_traffic(wname):
     return out
 
 
+def max_over_ranks(x, world, device):
+    """Max of a per-rank scalar over all ranks (torch.distributed all_reduce MAX; nccl on cuda, gloo on cpu)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def throughput_mpts(points_per_rank, steps, world, seconds):
+    """Whole-job Mpoints/s: points of all ranks x steps / (1e6 x max-over-ranks time)."""
+    return points_per_rank * steps * world / seconds / 1e6
+
+
 class ClockSampler:
     Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
@@ -244,10 +261,7 @@ def main():
     # per-kernel durations, CUDA events on the launching stream, same K steps of the same state
     prof = sim.step_profiled(K)
     clocks = sampler.stop() if sampler else None
-    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms = float(t.item())
+    ms = max_over_ranks(ms, world, "cuda")
     sim.destroy()
     del sim
     torch.cuda.empty_cache()
@@ -270,12 +284,9 @@ def main():
         sim.get_field_into(binding.FDTD_P, out_host.data_ptr())
         torch.cuda.synchronize()
         dt_e = time.perf_counter() - t0
-        tt = torch.tensor([dt_e], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        dt_e = float(tt.item())
+        dt_e = max_over_ranks(dt_e, world, "cuda")
         h2d = (n * 4 if c_host is not None else 0) + w.sources.nbytes + w.wavelets.nbytes
-        e2e = {"value": n * K * world / dt_e / 1e6, "unit": UNIT, "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": n * 4 / K,
+        e2e = {"value": throughput_mpts(n, K, world, dt_e), "unit": UNIT, "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": n * 4 / K,
                "seconds": dt_e, "what": "fdtd_set_model + fdtd_set_sources + fdtd_step(K) + fdtd_get_field(p), pinned host buffers"}
         sim.destroy()
         del sim
@@ -285,7 +296,7 @@ def main():
             dist.destroy_process_group()
         return 0
 
-    value = w.points * K * world / (ms * 1e-3) / 1e6
+    value = throughput_mpts(w.points, K, world, ms * 1e-3)
     bv, bp = algorithmic_bytes(w)
     peak, peak_src = peaks()
     dom = "update_v_tiled" if prof["update_v"] >= prof["update_p"] else "update_p_tiled"
