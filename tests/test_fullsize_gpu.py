@@ -27,11 +27,12 @@ def B():
 
 
 def _windows(total):
-    """Window origins: low corner, high corner, centre, the middle of the x-high face, a y-low / z-high edge."""
+    """Window origins: low corner, high corner, centre, the middle of the x-high face, a y-low / z-high edge, an odd
+    (tile-straddling) spot on the y-high face.  A window either contains a face or stays clear of that face's layer."""
     n = total
     mid = [(t - W) // 2 for t in n]
     hi = [t - W for t in n]
-    return [(0, 0, 0), tuple(hi), tuple(mid), (hi[0], mid[1], mid[2]), (mid[0], 0, hi[2]), (3, hi[1] - 5, mid[2] + 7)]
+    return [(0, 0, 0), tuple(hi), tuple(mid), (hi[0], mid[1], mid[2]), (mid[0], 0, hi[2]), (41, hi[1], mid[2] + 7)]
 
 
 def _check(B, w, sim):
