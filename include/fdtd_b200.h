@@ -40,7 +40,12 @@ enum { FDTD_PSI_VX = 0, FDTD_PSI_VY = 1, FDTD_PSI_VZ = 2, FDTD_PSI_PX = 3, FDTD_
 enum { FDTD_WALL = 0, FDTD_PERIODIC = 1 };
 enum {
   FDTD_KERNEL_AUTO = 0, /* TMA-staged, z-streaming tile kernels (the product path)                        */
-  FDTD_KERNEL_REF = 1   /* one thread per point, global loads only; also the only path for FDTD_PERIODIC   */
+  FDTD_KERNEL_REF = 1,  /* one thread per point, global loads only; also the only path for FDTD_PERIODIC   */
+  FDTD_KERNEL_FUSED = 2 /* one launch per time step: both sub-updates in a single pass over the fields (32 B  */
+                        /* per point instead of 48), the single-GPU form of the enlarged ghost of P:42 (a     */
+                        /* ghost of 2r = 8 cells per step, recomputed in x and y, streamed in z).  Out of      */
+                        /* place: the workspace holds two copies of the fields and psi.  Same bits as AUTO.   */
+                        /* Needs FDTD_WALL, total Nx % 4 == 0 and an even substeps_per_exchange.              */
 };
 
 /* Problem statement and Table 2 as one plain-data block. */
@@ -58,7 +63,7 @@ typedef struct {
                           /* pencil-yz keeps x local                                                  */
   int32_t ghost;          /* ghost depth g in cells on every internal interface                 */
   int32_t substeps_per_exchange; /* m sub-updates (v or p) between halo exchanges; needs g >= 4 m (R20)      */
-  int32_t kernel;         /* FDTD_KERNEL_AUTO / FDTD_KERNEL_REF                                              */
+  int32_t kernel;         /* FDTD_KERNEL_AUTO / FDTD_KERNEL_REF / FDTD_KERNEL_FUSED                          */
   int32_t device;         /* CUDA device ordinal                                                             */
   void* stream;           /* cudaStream_t the work is enqueued on (0 = legacy default stream)                */
   void* workspace;        /* DEVICE memory, 256-byte aligned, owned by the caller, must outlive the context  */
@@ -96,7 +101,8 @@ int fdtd_step(fdtd_ctx* ctx, int32_t n);
 
 /* fdtd_step with CUDA events recorded on params.stream around every launch group: out_ms_host[0] = total time of
  * the velocity sub-update kernels, [1] = pressure sub-update kernels, [2] = source injection, [3] = halo exchange,
- * in milliseconds over the n steps.  Same arithmetic and launches as fdtd_step.  Synchronises. */
+ * in milliseconds over the n steps (FDTD_KERNEL_FUSED: [0] = the fused step kernel, [1] = 0).  Same arithmetic and
+ * launches as fdtd_step.  Synchronises. */
 int fdtd_step_profiled(fdtd_ctx* ctx, int32_t n, double out_ms_host[4]);
 
 /* Copies one field (FDTD_P..FDTD_VZ) of the total grid, unpadded, to dst_host (Nz*Ny*Nx fp32).  In subdomain

@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libfdtd_b200.so")
 FDTD_P, FDTD_VX, FDTD_VY, FDTD_VZ = 0, 1, 2, 3
 FDTD_PSI_VX, FDTD_PSI_VY, FDTD_PSI_VZ, FDTD_PSI_PX, FDTD_PSI_PY, FDTD_PSI_PZ = range(6)
 FDTD_WALL, FDTD_PERIODIC = 0, 1
-FDTD_KERNEL_AUTO, FDTD_KERNEL_REF = 0, 1
+FDTD_KERNEL_AUTO, FDTD_KERNEL_REF, FDTD_KERNEL_FUSED = 0, 1, 2
 FDTD_OK, FDTD_EINVAL, FDTD_EWORKSPACE, FDTD_ECUDA, FDTD_EUNSUPPORTED = 0, -1, -2, -3, -4
 
 # every symbol include/fdtd_b200.h declares

@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfdtd_b200.so")
 SOURCES = [os.path.join(CSRC, "fdtd_b200.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "fdtd_kernels.cuh"), os.path.join(HERE, "..", "include", "fdtd_b200.h")]
+DEPS = SOURCES + [os.path.join(CSRC, "fdtd_kernels.cuh"), os.path.join(CSRC, "fdtd_fused.cuh"), os.path.join(HERE, "..", "include", "fdtd_b200.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "-Xptxas", "-v",

@@ -3,6 +3,7 @@
 // (P:76-82).  No CPU fallback: every compute entry point needs a CUDA device.
 #include "../../include/fdtd_b200.h"
 #include "fdtd_kernels.cuh"
+#include "fdtd_fused.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -69,6 +70,8 @@ struct Geometry {
   std::string why;
 };
 
+long long n_total_x(const fdtd_params& P) { return (long long)P.n_interior[0] + P.cpml[0] + P.cpml[1]; }
+
 Geometry make_geometry(const fdtd_params& P) {
   Geometry G;
   auto bad = [&](const char* w) { G.valid = false; G.why = w; return G; };
@@ -82,6 +85,9 @@ Geometry make_geometry(const fdtd_params& P) {
   }
   if (!(P.dx > 0.0) || !(P.dt > 0.0)) return bad("dx and dt must be positive");
   if (P.boundary != FDTD_WALL && P.boundary != FDTD_PERIODIC) return bad("unknown boundary");
+  if (P.kernel < FDTD_KERNEL_AUTO || P.kernel > FDTD_KERNEL_FUSED) return bad("unknown kernel selector");
+  if (P.kernel == FDTD_KERNEL_FUSED && (P.boundary == FDTD_PERIODIC || (n_total_x(P) % 4) != 0))
+    return bad("FDTD_KERNEL_FUSED needs WALL boundaries and a total Nx that is a multiple of 4");
   if (P.boundary == FDTD_PERIODIC)
     for (int f = 0; f < 6; ++f) if (P.cpml[f]) return bad("PERIODIC excludes CPML");
   for (int f = 0; f < 6; ++f)
@@ -94,6 +100,7 @@ Geometry make_geometry(const fdtd_params& P) {
   if (sub) {
     if (P.boundary == FDTD_PERIODIC) return bad("subdomain mode needs WALL boundaries");
     if (G.msub < 1 || G.ghost < 4 * G.msub) return bad("ghost must be >= 4 * substeps_per_exchange");
+    if (P.kernel == FDTD_KERNEL_FUSED && (G.msub % 2)) return bad("the fused step advances two sub-updates: substeps_per_exchange must be even");
     for (int a = 1; a < 3; ++a) {
       if (G.gn[a] % G.nd[a]) return bad("total grid not divisible by decomp");
       if (G.gn[a] / G.nd[a] < G.ghost) return bad("ghost deeper than a subdomain");
@@ -117,8 +124,12 @@ struct Domain {
   int own_lo[3], own_hi[3];    // owned cells in local indices
   int cy, cz;                  // position in the subdomain grid
   TMaps tm;
-  unsigned int* counters = nullptr;  // device: [0] update_v work counter, [1] update_p work counter
+  OutSet alt;                  // fused mode: the other state (fields + psi); swapped with v.f / v.psi after every launch
+  TMaps tm_alt;                // its tensor maps
+  unsigned int* counters = nullptr;  // device: [0] update_v, [1] update_p, [2], [3] step_fused (alternating) work counters
   Sched sched;
+  Sched sched_f;               // work decomposition of step_fused
+  int fused_parity = 0;
   long long* src_offset = nullptr;   // device, per source
 };
 
@@ -128,6 +139,7 @@ struct Layout {
     int n[3], o[3], pitch;
     int ls[3][2], ln[3][2];
     uint64_t f[4], kc, psi[2][3][2], src_off, counters;
+    uint64_t f2[4], psi2[2][3][2];   // fused mode: second state
   };
   std::vector<Dom> doms;
   uint64_t tab[2][3][3];
@@ -172,6 +184,15 @@ Layout make_layout(const fdtd_params& P, const Geometry& G) {
           d.psi[fam][1][s] = take((uint64_t)d.pitch * d.ln[1][s] * d.n[2] * 4 + 16);
           d.psi[fam][2][s] = take((uint64_t)d.pitch * d.n[1] * d.ln[2][s] * 4 + 16);
         }
+      if (P.kernel == FDTD_KERNEL_FUSED) {
+        for (int f = 0; f < 4; ++f) d.f2[f] = take(vol);
+        for (int fam = 0; fam < 2; ++fam)
+          for (int s = 0; s < 2; ++s) {
+            d.psi2[fam][0][s] = take((uint64_t)d.ln[0][s] * d.n[1] * d.n[2] * 4 + 16);
+            d.psi2[fam][1][s] = take((uint64_t)d.pitch * d.ln[1][s] * d.n[2] * 4 + 16);
+            d.psi2[fam][2][s] = take((uint64_t)d.pitch * d.n[1] * d.ln[2][s] * 4 + 16);
+          }
+      }
       d.src_off = take(MAX_SRC * sizeof(long long));
       d.counters = take(64);
       L.doms.push_back(d);
@@ -215,6 +236,8 @@ struct fdtd_ctx {
   AxisTable tabs[2][3];
   std::vector<float> dev_a[2][3];
   bool use_ref;
+  bool fused = false;
+  int grid_f = 0;
   int nsrc = 0, wlen = 0;
   long long* d_step;
   float* d_wav;
@@ -237,9 +260,9 @@ int make_tmap(EncodeTiledFn enc, CUtensorMap* m, float* base, const DomainView& 
 }
 
 // Persistent launch plan: grid = resident CTAs; items = tiles x z-chunks with enough items per CTA for balance.
-int plan_launch(fdtd_ctx* c, const void* kernel, int smem, int* grid) {
+int plan_launch(fdtd_ctx* c, const void* kernel, int smem, int* grid, int threads = NT) {
   int per_sm = 0, sms = 148;
-  CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, NT, smem));
+  CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem));
   CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->P.device));
   if (per_sm < 1) { set_err("tiled kernel does not fit on an SM"); return FDTD_ECUDA; }
   if (const char* e = getenv("FDTD_CTAS_PER_SM")) per_sm = std::max(1, std::min(per_sm, atoi(e)));
@@ -261,6 +284,39 @@ void plan_items(Domain& d, int grid) {
   S.zchunk = (v.nz + n - 1) / n;
   S.nzc = (v.nz + S.zchunk - 1) / S.zchunk;
   S.nitems = (int)(tiles * S.nzc);
+}
+
+// step_fused items: the z lead-in of an item is 14 planes (7 of them load only a p tile), so chunks are long.
+void plan_items_fused(Domain& d, int grid) {
+  const DomainView& v = d.v;
+  Sched& S = d.sched_f;
+  S.ntx = (v.nx + TX - 1) / TX;
+  S.nty = (v.ny + TY - 1) / TY;
+  const long long tiles = (long long)S.ntx * S.nty;
+  long long zc = (long long)v.nz * tiles / (6LL * std::max(grid, 1));
+  zc = std::max(32LL, std::min(256LL, zc));
+  if (const char* e = getenv("FDTD_ZCHUNK_FUSED")) zc = std::max(1, atoi(e));
+  int n = (int)((v.nz + zc - 1) / zc);
+  S.zchunk = (v.nz + n - 1) / n;
+  S.nzc = (v.nz + S.zchunk - 1) / S.zchunk;
+  S.nitems = (int)(tiles * S.nzc);
+}
+
+// One fused time step of one domain: state v.f / v.psi -> d.alt, then the two are swapped.
+int launch_fused(fdtd_ctx* c, Domain& d) {
+  Sched S = d.sched_f;
+  S.counter = d.counters + 2 + d.fused_parity;
+  S.other = d.counters + 2 + (1 - d.fused_parity);
+  step_fused<<<std::min(c->grid_f, S.nitems), FNT, F_SMEM_BYTES, c->stream>>>(d.tm, d.v, d.alt, S);
+  c->launches++;
+  CK(cudaGetLastError());
+  d.fused_parity ^= 1;
+  for (int f = 0; f < 4; ++f) std::swap(d.v.f[f], d.alt.f[f]);
+  for (int fam = 0; fam < 2; ++fam)
+    for (int a = 0; a < 3; ++a)
+      for (int s = 0; s < 2; ++s) std::swap(d.v.psi[fam][a][s], d.alt.psi[fam][a][s]);
+  std::swap(d.tm, d.tm_alt);
+  return FDTD_OK;
 }
 
 int launch_substep(fdtd_ctx* c, Domain& d, int which /*0 = v, 1 = p*/) {
@@ -410,6 +466,19 @@ int exchange_halos(fdtd_ctx* c) {
   return FDTD_OK;
 }
 
+int do_fused_step(fdtd_ctx* c) {
+  if (c->doms.size() > 1 && c->substeps_done % c->G.msub == 0) {
+    int r = exchange_halos(c);
+    if (r) return r;
+  }
+  for (auto& d : c->doms) {
+    int r = launch_fused(c, d);
+    if (r) return r;
+  }
+  c->substeps_done += 2;
+  return FDTD_OK;
+}
+
 int do_substep(fdtd_ctx* c, int which) {
   if (c->doms.size() > 1 && c->substeps_done % c->G.msub == 0) {
     int r = exchange_halos(c);
@@ -491,6 +560,7 @@ fdtd_ctx* fdtd_create(const fdtd_params* P) {
   c->stream = (cudaStream_t)P->stream;
   // the tiled kernels move whole float4s: they need Nx % 4 == 0; other grids take the reference kernels
   c->use_ref = P->kernel == FDTD_KERNEL_REF || P->boundary == FDTD_PERIODIC || (G.gn[0] % 4) != 0;
+  c->fused = P->kernel == FDTD_KERNEL_FUSED;      // make_geometry has checked that the tiled path applies
   cudaError_t e;
   if ((e = cudaSetDevice(P->device)) != cudaSuccess) return fail(c, e, "cudaSetDevice");
   if ((e = cudaMemsetAsync(c->ws, 0, L.total, c->stream)) != cudaSuccess) return fail(c, e, "cudaMemsetAsync(workspace)");
@@ -556,10 +626,21 @@ fdtd_ctx* fdtd_create(const fdtd_params* P) {
       d.counters = (unsigned int*)(c->ws + ld.counters);
       if (!c->use_ref) {
         float* kcbase = (float*)(c->ws + ld.kc);
-        float* tile_base[5] = {v.f[0], v.f[1], v.f[2], v.f[3], kcbase};
-        int bad = make_tmap(enc, &d.tm.p_halo, v.f[0], v, HW, VH) || make_tmap(enc, &d.tm.vx_halo, v.f[1], v, HW, TY) ||
-                  make_tmap(enc, &d.tm.vy_halo, v.f[2], v, TX, PH);
-        for (int t = 0; t < 5 && !bad; ++t) bad = make_tmap(enc, &d.tm.tile[t], tile_base[t], v, TX, TY);
+        auto make_maps = [&](TMaps& tm, float* const f[4]) -> int {
+          float* tile_base[5] = {f[0], f[1], f[2], f[3], kcbase};
+          int bad = make_tmap(enc, &tm.p_halo, f[0], v, HW, VH) || make_tmap(enc, &tm.vx_halo, f[1], v, HW, TY) ||
+                    make_tmap(enc, &tm.vy_halo, f[2], v, TX, PH) || make_tmap(enc, &tm.p_box, f[0], v, BW, BH);
+          for (int t = 0; t < 5 && !bad; ++t) bad = make_tmap(enc, &tm.tile[t], tile_base[t], v, TX, TY);
+          return bad;
+        };
+        int bad = make_maps(d.tm, v.f);
+        if (c->fused && !bad) {
+          for (int f = 0; f < 4; ++f) d.alt.f[f] = (float*)(c->ws + ld.f2[f]);
+          for (int fam = 0; fam < 2; ++fam)
+            for (int a = 0; a < 3; ++a)
+              for (int s = 0; s < 2; ++s) d.alt.psi[fam][a][s] = (float*)(c->ws + ld.psi2[fam][a][s]);
+          bad = make_maps(d.tm_alt, d.alt.f);
+        }
         if (bad) { delete c; return nullptr; }
       }
       c->doms.push_back(d);
@@ -573,6 +654,12 @@ fdtd_ctx* fdtd_create(const fdtd_params* P) {
     if (plan_launch(c, (const void*)update_v_tiled, V_SMEM_BYTES, &c->grid_v) ||
         plan_launch(c, (const void*)update_p_tiled, P_SMEM_BYTES, &c->grid_p)) { delete c; return nullptr; }
     for (auto& d : c->doms) plan_items(d, std::min(c->grid_v, c->grid_p));
+    if (c->fused) {
+      if ((e = cudaFuncSetAttribute(step_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, F_SMEM_BYTES)) != cudaSuccess)
+        return fail(c, e, "cudaFuncSetAttribute(step_fused)");
+      if (plan_launch(c, (const void*)step_fused, F_SMEM_BYTES, &c->grid_f, FNT)) { delete c; return nullptr; }
+      for (auto& d : c->doms) plan_items_fused(d, c->grid_f);
+    }
   }
   return c;
 }
@@ -648,8 +735,12 @@ int fdtd_step(fdtd_ctx* c, int32_t n) {
   if (!c || n < 0) return FDTD_EINVAL;
   for (int s = 0; s < n; ++s) {
     int r;
-    if ((r = do_substep(c, 0))) return r;     // velocity sub-update
-    if ((r = do_substep(c, 1))) return r;     // pressure sub-update
+    if (c->fused) {
+      if ((r = do_fused_step(c))) return r;   // both sub-updates in one pass (a7)
+    } else {
+      if ((r = do_substep(c, 0))) return r;   // velocity sub-update
+      if ((r = do_substep(c, 1))) return r;   // pressure sub-update
+    }
     if ((r = launch_inject(c))) return r;     // source (R14)
   }
   return FDTD_OK;
@@ -671,7 +762,16 @@ int fdtd_step_profiled(fdtd_ctx* c, int32_t n, double out_ms[4]) {
   };
   r = mark(-1);
   for (int s = 0; s < n && !r; ++s) {
-    for (int which = 0; which < 2 && !r; ++which) {
+    if (c->fused) {
+      if (c->doms.size() > 1 && c->substeps_done % c->G.msub == 0) {
+        r = exchange_halos(c);
+        if (!r) r = mark(3);
+      }
+      for (auto& d : c->doms) if (!r) r = launch_fused(c, d);
+      c->substeps_done += 2;
+      if (!r) r = mark(0);
+    }
+    for (int which = 0; which < 2 && !r && !c->fused; ++which) {
       if (c->doms.size() > 1 && c->substeps_done % c->G.msub == 0) {
         r = exchange_halos(c);
         if (!r) r = mark(3);

@@ -201,6 +201,7 @@ struct TMaps {
   CUtensorMap vx_halo;    // vx, box HW x TY   (update_p)
   CUtensorMap vy_halo;    // vy, box TX x PH   (update_p)
   CUtensorMap tile[5];    // p, vx, vy, vz, kc with box TX x TY
+  CUtensorMap p_box;      // p,  box (TX+16) x (TY+14)   (step_fused)
 };
 
 // Work decomposition of one launch (same for both sub-updates of a domain).

@@ -21,13 +21,15 @@ def test_byte_models_match_survey_8d():
     # two-pass model 48 B/pt + psi 16 B per slab point per axis (+4 for a Kc array): SURVEY 8d / BASELINE.md table
     for idx, expect in ((2, 53.33), (4, 49.92)):
         w = inputs.config(idx, steps=1)
-        bv, bp = bench.algorithmic_bytes(w)
+        bv, bp, bf = bench.algorithmic_bytes(w)
         assert abs((bv + bp) / w.points - expect) < 0.01
+        assert abs(bf / w.points - (expect - 16.0)) < 0.01        # single pass: 32 instead of 48 B/pt, same psi bytes
     w = inputs.config(1, steps=1)
-    bv, bp = bench.algorithmic_bytes(w)
+    bv, bp, bf = bench.algorithmic_bytes(w)
     assert bv == 28 * 80 ** 3 + 8 * 3 * 16 * 80 * 80 and bp == 20 * 80 ** 3 + 8 * 3 * 16 * 80 * 80
-    w.c = 1                                  # a Kc array adds 4 B/pt to update_p only
-    assert bench.algorithmic_bytes(w)[1] == bp + 4 * 80 ** 3
+    assert bf == 32 * 80 ** 3 + 16 * 3 * 16 * 80 * 80
+    w.c = 1                                  # a Kc array adds 4 B/pt to update_p and to the fused step
+    assert bench.algorithmic_bytes(w)[1] == bp + 4 * 80 ** 3 and bench.algorithmic_bytes(w)[2] == bf + 4 * 80 ** 3
     assert bench.throughput_mpts(1000, 10, 2, 0.5) == pytest.approx(1000 * 10 * 2 / 0.5 / 1e6)
 
 

@@ -49,7 +49,7 @@ def test_coefficients_and_cpml_tables_match_oracle(B):
     sim.destroy()
 
 
-@pytest.mark.parametrize("kernel", [1, 0])
+@pytest.mark.parametrize("kernel", [1, 0, 2])
 def test_config1_full_parity(B, kernel):
     """BASELINE config 1 in full: 64^3 + 8-cell CPML, centre Ricker source, 100 steps, zero initial fields."""
     w = inputs.config(1)
@@ -69,7 +69,7 @@ def test_config1_full_parity(B, kernel):
     sim.destroy()
 
 
-@pytest.mark.parametrize("kernel", [1, 0])
+@pytest.mark.parametrize("kernel", [1, 0, 2])
 @pytest.mark.parametrize("shape,cpml", [
     ((70, 45, 37), (5, 9, 0, 7, 6, 0)),        # ragged tiles in x and y, faces without a layer, unequal thickness
     ((133, 18, 21), (12, 12, 4, 4, 8, 8)),     # nx not a multiple of 4: the library routes this to the reference kernels
@@ -79,6 +79,8 @@ def test_config1_full_parity(B, kernel):
 def test_random_state_ragged_parity(B, kernel, shape, cpml):
     """All four fields random (counter-based generator on both sides), heterogeneous c, 6 steps."""
     tot = tuple(shape[a] + cpml[2 * a] + cpml[2 * a + 1] for a in range(3))
+    if kernel == 2 and tot[0] % 4:
+        pytest.skip("FDTD_KERNEL_FUSED needs Nx % 4 == 0 (fdtd_create refuses, see test_errors_are_reported_not_fatal)")
     rng = np.random.default_rng(11)
     c = (1.0 + 0.3 * rng.random(tot[::-1])).astype(np.float32)
     kw = dict(dt=0.4 / 1.3, cpml_alpha_max=math.pi * inputs.F0, cpml_c_ref=1.3)
@@ -117,6 +119,37 @@ def test_tiled_and_reference_kernels_agree_bitwise(B):
         sim.destroy()
     for a, b in zip(*out):
         assert np.array_equal(a, b)
+
+
+@pytest.mark.parametrize("shape,cpml,het", [
+    ((92, 40, 33), (8, 8, 8, 8, 8, 8), False),
+    ((180, 50, 90), (12, 12, 20, 20, 9, 9), True),     # 4 x tiles, 6 y tiles, CPML wider than a y tile, Kc array
+    ((58, 28, 300), (0, 6, 5, 0, 16, 3), True),        # several z chunks, faces without a layer
+])
+def test_fused_and_two_pass_agree_bitwise(B, shape, cpml, het):
+    """a7: the single-pass step (one launch, out of place) gives the bits of update_v followed by update_p."""
+    tot = tuple(shape[a] + cpml[2 * a] + cpml[2 * a + 1] for a in range(3))
+    kw = dict(dt=0.4 / 1.3, cpml_alpha_max=math.pi * inputs.F0, cpml_c_ref=1.3)
+    c = (1.0 + 0.3 * np.random.default_rng(5).random(tot[::-1])).astype(np.float32) if het else None
+    src = np.array([[tot[0] // 2, tot[1] // 3, tot[2] // 2], [3, 2, 1]], np.int32)
+    wav = np.stack([inputs.ricker(7, kw["dt"], t0=1.0), 0.1 * np.ones(7, np.float32)])
+    out = []
+    for kernel in (0, 2):
+        sim = B.Fdtd(shape, cpml, kernel=kernel, **kw)
+        if het:
+            sim.set_model(c)
+        sim.set_sources(src, wav)
+        for f in range(4):
+            sim.fill_hash(f, 7, 1.0)
+        sim.step(3)
+        mid = [sim.get_field(f) for f in range(4)]                 # odd number of swaps
+        sim.step(4)
+        if kernel == 2:
+            assert sim.launch_count() == 4 + int(het) + 2 * 7      # fills (+ Kc) + (one fused launch + one inject) per step
+        out.append(mid + [sim.get_field(f) for f in range(4)] + [sim.get_psi(q) for q in range(6)])
+        sim.destroy()
+    for n, (a, b) in enumerate(zip(*out)):
+        assert np.array_equal(a.view(np.uint32), b.view(np.uint32)), n
 
 
 def test_periodic_dispersion_on_gpu(B):
@@ -176,3 +209,6 @@ def test_errors_are_reported_not_fatal(B):
         sim.set_model(None, rho)
     sim.step(1)
     sim.destroy()
+    for bad in (dict(n_interior=(18, 16, 16)), dict(n_interior=(16,) * 3, boundary=B.FDTD_PERIODIC)):
+        with pytest.raises(B.FdtdError):                            # the fused step refuses what it cannot run
+            B.Fdtd(bad.pop("n_interior"), dt=0.4, kernel=B.FDTD_KERNEL_FUSED, **bad)

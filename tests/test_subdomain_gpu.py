@@ -50,6 +50,20 @@ def test_subdomains_bit_identical_small(B, kernel, g, m):
     assert launches > 24 * 2 * 4                                # 4 subdomains x 2 sub-updates per step + exchanges
 
 
+@pytest.mark.parametrize("g,m", [(8, 2), (16, 4), (12, 2), (32, 8)])
+def test_subdomains_bit_identical_fused(B, g, m):
+    """The fused single-pass step inside every subdomain (two sub-updates per launch, so m is even): same bits as the
+    monolithic two-kernel run."""
+    shape, cpml = (72, 80, 88), (8, 8, 8, 8, 8, 8)
+    src = [(44, 48, 52), (5, 47, 51), (80, 60, 20)]
+    ref, _ = _run(B, shape, cpml, 24, True, src, kernel=0)
+    sub, _ = _run(B, shape, cpml, 24, True, src, kernel=2, decomp=(1, 2, 2), ghost=g, substeps=m)
+    for a, b in zip(ref, sub):
+        assert _same_bits(a, b), float(np.abs(a - b).max())
+    with pytest.raises(B.FdtdError):
+        B.Fdtd(shape, cpml, dt=0.4, kernel=2, decomp=(1, 2, 2), ghost=4, substeps=1)   # odd m cannot be fused
+
+
 def test_insufficient_ghost_is_rejected(B):
     with pytest.raises(B.FdtdError):
         B.Fdtd((64,) * 3, (8,) * 6, dt=0.4, decomp=(1, 2, 2), ghost=8, substeps=3)
