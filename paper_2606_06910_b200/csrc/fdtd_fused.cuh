@@ -340,20 +340,31 @@ __global__ void __launch_bounds__(FNT, 1) step_fused(const __grid_constant__ TMa
     if (blockIdx.x == 0) *S.other = 0u;
   }
   const int warp = threadIdx.x >> 5;
-  const bool has_kc = D.kc != nullptr;
   unsigned it = 0, eit = 0;
   int x0, y0, z0, z1;
-  while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) {
-    const int niter = z1 - z0 + 14, nout = z1 - z0;
-    if (threadIdx.x == FW_MAIN * 32) {
-#pragma unroll
-      for (int s = 0; s < FNS; ++s)
-        if (s < niter) fused_issue(tm, smem, Q.full, (it + s) % FNS, z0 - 7 + s, x0, y0, z0, has_kc);
+  // The two roles never share code after this point, so each is compiled against its own register budget: the two main
+  // warpgroups take the registers the halo warpgroup gives up (3 warps per SM sub-partition: 2 x 216 + 72 <= 512).
+  if (warp < FW_MAIN) {
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(F_REGS_MAIN));
+    while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) {
+      fused_main(D, O, smem, ebuf, Q, it, eit, x0, y0, z0, z1);
+      it += z1 - z0 + 14;
+      eit += z1 - z0;
     }
-    if (warp < FW_MAIN) fused_main(D, O, smem, ebuf, Q, it, eit, x0, y0, z0, z1);
-    else fused_halo(tm, D, smem, ebuf, Q, it, eit, warp - FW_MAIN, x0, y0, z0, z1);
-    it += niter;
-    eit += nout;
+  } else {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(F_REGS_HALO));
+    const bool has_kc = D.kc != nullptr;
+    while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) {
+      const int niter = z1 - z0 + 14;
+      if (threadIdx.x == FW_MAIN * 32) {
+#pragma unroll
+        for (int s = 0; s < FNS; ++s)
+          if (s < niter) fused_issue(tm, smem, Q.full, (it + s) % FNS, z0 - 7 + s, x0, y0, z0, has_kc);
+      }
+      fused_halo(tm, D, smem, ebuf, Q, it, eit, warp - FW_MAIN, x0, y0, z0, z1);
+      it += niter;
+      eit += z1 - z0;
+    }
   }
 }
 
