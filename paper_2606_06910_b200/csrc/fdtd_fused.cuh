@@ -57,7 +57,6 @@ struct FusedBars {
   uint64_t* full;     // [FNS] TMA stage landed
   uint64_t* empty;    // [FNS] every warp has read the stage
   uint64_t* efull;    // [2]   every warp has written its part of the exchange buffer
-  uint64_t* eempty;   // [2]   every main warp has read the exchange buffer
 };
 
 __device__ __forceinline__ void warp_arrive(uint64_t* bar) {
@@ -84,149 +83,215 @@ __device__ __forceinline__ void fused_issue(const TMaps& tm, float* smem, uint64
 }
 
 // ---- main warps: the tile's own points ------------------------------------------------------------------
-__device__ __forceinline__ void fused_main(const DomainView& D, const OutSet& O, const float* smem, float* ebuf, const FusedBars& Q,
-                                           unsigned it, unsigned eit, int x0, int y0, int z0, int z1) {
-  const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
-  const int i = x0 + 4 * tx, j = y0 + ty;
-  const bool has_kc = D.kc != nullptr;
-  const bool active = (i < D.nx) && (j < D.ny);
-  const float B = D.b0;
-  const float Bxy = active ? B : 0.f;
-  const float Bx3 = (i + 3 + D.ox) == D.gn[0] - 1 ? 0.f : Bxy;           // pinned last half node (R3)
-  const float By = (j + D.oy) == D.gn[1] - 1 ? 0.f : Bxy;
-  const long long rowoff = (long long)j * D.pitch + i;
-  long long goff = rowoff + (long long)z0 * D.plane;                     // plane k  (vx, vy, p)
-  long long goffz = rowoff + (long long)(z0 - 4) * D.plane;              // plane kz (vz); first used at kz = z0-4
-  const int boff = (ty + 7) * BW + 4 * tx + 8;                           // own float4 in the p box
-  const int toff = ty * TX + 4 * tx;                                     // own float4 in a plain tile
-  const int exo = ty * HW + 4 * tx + 4;                                  // own float4 in E.vx
-  const int eyo = E_OFF_VY + (ty + 4) * TX + 4 * tx;                     // own float4 in E.vy
-  const bool any_x = touches(D, 0, x0, x0 + TX), any_y = touches(D, 1, y0, y0 + TY);
-  const int sx = (any_x && active) ? slab_side(D, 0, i) : -1;
-  const int sy = (any_y && active) ? slab_side(D, 1, j) : -1;
-  long long pox = sx >= 0 ? psi_index(D, 0, sx, i, j, z0) : 0;           // same offset in psi_v / psi_p, in / out
-  long long poy = sy >= 0 ? psi_index(D, 1, sy, i, j, z0) : 0;
-  const long long stride_px = sx >= 0 ? (long long)D.ny * D.ln[0][sx] : 0;
-  const long long stride_py = sy >= 0 ? (long long)D.ln[1][sy] * D.pitch : 0;
-  const int gi = i + D.ox, gj = j + D.oy;
+// Per-thread state of a main thread over one item.  The two z queues are arrays that are only ever indexed with
+// compile-time constants (the steady loop is unrolled 8x so that the rotation is a renaming, not a move).
+struct MainCtx {
+  V4 pq[8];                 // p_old ring:  canonical order pq[n] = p_old[m-7+n]
+  V4 wq[8];                 // vz_new ring: canonical order wq[n] = vz_new[kz-7+n]
+  float* gvx; float* gvy; float* gvz; float* gp;      // output pointers of the current planes (k, k, kz, k)
+  long long pox, poy;       // psi offsets of plane k in the x / y slab arrays (same in psi_v / psi_p, in / out)
+  V4 nvx, nvy, npx, npy;    // psi_v / psi_p of plane k, loaded one iteration ahead (items that touch an x / y slab)
+  unsigned it, eit;
+};
 
-  V4 q0 = zero4(), q1 = zero4(), q2 = zero4(), q3 = zero4(), q4 = zero4(), q5 = zero4(), q6 = zero4(), q7 = zero4();   // p_old[m-7 .. m]
-  V4 w0 = zero4(), w1 = zero4(), w2 = zero4(), w3 = zero4(), w4 = zero4(), w5 = zero4(), w6 = zero4(), w7 = zero4();   // vz_new[kz-7 .. kz]
+struct MainConst {
+  int i, j, tx, ty, boff, toff, exo, eyo, sx, sy, gi, gj, z0, z1, zl, zh;
+  long long stride_px, stride_py, zrow;
+  float Bxy, Bx3, By;
+  bool active, has_kc;
+};
 
-  for (int m = z0 - 7; m < z1 + 7; ++m, ++it) {
-    const unsigned slot = it % FNS;
-    const int k = m - 7, kz = m - 4;
-    const bool out = k >= z0, hvz = m >= z0;
-    const float* st = smem + slot * F_STAGE_FLOATS;
-    // psi of the velocity family: issue the global loads before waiting on the tile
-    V4 psx, psy, psz;
-    const int szv = (hvz && active && kz >= 0 && kz < D.nz) ? slab_side(D, 2, kz) : -1;
-    long long poz = 0;
-    if (out && sx >= 0) psx = ldg4(D.psi[0][0][sx] + pox);
-    if (out && sy >= 0) psy = ldg4(D.psi[0][1][sy] + poy);
-    if (szv >= 0) { poz = psi_index(D, 2, szv, i, j, kz); psz = ldg4(D.psi[0][2][szv] + poz); }
-    // ... and of the pressure family at plane k
-    const int szp = (out && active) ? slab_side(D, 2, k) : -1;
-    V4 ppx, ppy, ppz;
-    long long pozp = 0;
-    if (out && sx >= 0) ppx = ldg4(D.psi[1][0][sx] + pox);
-    if (out && sy >= 0) ppy = ldg4(D.psi[1][1][sy] + poy);
-    if (szp >= 0) { pozp = psi_index(D, 2, szp, i, j, k); ppz = ldg4(D.psi[1][2][szp] + pozp); }
-
-    mbar_wait(&Q.full[slot], (it / FNS) & 1);
-    q0 = q1; q1 = q2; q2 = q3; q3 = q4; q4 = q5; q5 = q6; q6 = q7; q7 = ld4(st + F_OFF_PT + toff);
-    V4 dxv, dyv, vx4, vy4, vz4, kc4;
-    if (out) {
-      const float* row = st + boff;
-      const V4 c = ld4(row);
-      dxv = diff_x<true>(ld4(row - 4), c, ld4(row + 4));
-      dyv = diff_8(ld4(row + BW), c, ld4(row + 2 * BW), ld4(row - BW), ld4(row + 3 * BW), ld4(row - 2 * BW), ld4(row + 4 * BW),
-                   ld4(row - 3 * BW));
-      vx4 = ld4(st + F_OFF_VX + exo);
-      vy4 = ld4(st + F_OFF_VY + (ty + 4) * TX + 4 * tx);
-      kc4 = has_kc ? ld4(st + F_OFF_KC + toff) : splat4(D.kc0);
-    }
-    if (hvz) vz4 = ld4(st + F_OFF_VZ + toff);
-    warp_arrive(&Q.empty[slot]);
-
-    const unsigned eb = eit & 1, eu = eit >> 1;
-    float* E = ebuf + eb * E_FLOATS;
-    if (out) {
-      // ---- velocity sub-update at plane k
-      if (any_x) {
-        if (sx >= 0) {
-          cpml4(dxv, psx, ldg4(D.tab[0][0][0] + gi), ldg4(D.tab[0][0][1] + gi), ldg4(D.tab[0][0][2] + gi));
-          st4(O.psi[0][0][sx] + pox, psx);
-        }
-      }
-      if (any_y) {
-        if (sy >= 0) {
-          cpml4s(dyv, psy, __ldg(D.tab[0][1][0] + gj), __ldg(D.tab[0][1][1] + gj), __ldg(D.tab[0][1][2] + gj));
-          st4(O.psi[0][1][sy] + poy, psy);
-        }
-      }
-      vx4.v[0] = upd(vx4.v[0], Bxy, dxv.v[0]); vx4.v[1] = upd(vx4.v[1], Bxy, dxv.v[1]);
-      vx4.v[2] = upd(vx4.v[2], Bxy, dxv.v[2]); vx4.v[3] = upd(vx4.v[3], Bx3, dxv.v[3]);
+__device__ __forceinline__ void shift_push(V4 (&q)[8], const V4& v) {
 #pragma unroll
-      for (int e = 0; e < 4; ++e) vy4.v[e] = upd(vy4.v[e], By, dyv.v[e]);
-      if (active) { st4(O.f[1] + goff, vx4); st4(O.f[2] + goff, vy4); }
-      mbar_wait(&Q.eempty[eb], (eu & 1) ^ 1);            // the readers of two planes ago are done with this buffer
-      st4(E + exo, vx4);
-      st4(E + eyo, vy4);
-      warp_arrive(&Q.efull[eb]);
-    }
-    if (hvz) {
-      // ---- vz_new at kz+1/2 from p_old[kz-3 .. kz+4] = q0..q7
-      V4 dzv = diff_8(q4, q3, q5, q2, q6, q1, q7, q0);
-      const int gk = kz + D.oz;
-      if (szv >= 0) {
-        cpml4s(dzv, psz, __ldg(D.tab[0][2][0] + gk), __ldg(D.tab[0][2][1] + gk), __ldg(D.tab[0][2][2] + gk));
-        if (kz >= z0 && kz < z1) st4(O.psi[0][2][szv] + poz, psz);      // lead-in / tail planes belong to another item
-      }
-      const float Bz = (kz < 0 || kz >= D.nz || gk == D.gn[2] - 1) ? 0.f : Bxy;
-#pragma unroll
-      for (int e = 0; e < 4; ++e) vz4.v[e] = upd(vz4.v[e], Bz, dzv.v[e]);
-      if (active && kz >= z0 && kz < z1) st4(O.f[3] + goffz, vz4);
-      w0 = w1; w1 = w2; w2 = w3; w3 = w4; w4 = w5; w5 = w6; w6 = w7; w7 = vz4;
-      goffz += D.plane;
-    }
-    if (out) {
-      // ---- pressure sub-update at plane k: vz_new[k-4 .. k+3] = w0..w7
-      V4 dzp = diff_8(w4, w3, w5, w2, w6, w1, w7, w0);
-      mbar_wait(&Q.efull[eb], eu & 1);
-      const float* xr = E + exo;
-      V4 dxp = diff_x<false>(ld4(xr - 4), vx4, ld4(xr + 4));
-      const float* col = E + E_OFF_VY + ty * TX + 4 * tx;                 // row ty of E.vy <-> y = j-4
-      V4 dyp = diff_8(vy4, ld4(col + 3 * TX), ld4(col + 5 * TX), ld4(col + 2 * TX), ld4(col + 6 * TX), ld4(col + TX), ld4(col + 7 * TX),
-                      ld4(col));
-      warp_arrive(&Q.eempty[eb]);
-      if (any_x) {
-        if (sx >= 0) {
-          cpml4(dxp, ppx, ldg4(D.tab[1][0][0] + gi), ldg4(D.tab[1][0][1] + gi), ldg4(D.tab[1][0][2] + gi));
-          st4(O.psi[1][0][sx] + pox, ppx);
-          pox += stride_px;
-        }
-      }
-      if (any_y) {
-        if (sy >= 0) {
-          cpml4s(dyp, ppy, __ldg(D.tab[1][1][0] + gj), __ldg(D.tab[1][1][1] + gj), __ldg(D.tab[1][1][2] + gj));
-          st4(O.psi[1][1][sy] + poy, ppy);
-          poy += stride_py;
-        }
-      }
-      if (szp >= 0) {
-        const int gk = k + D.oz;
-        cpml4s(dzp, ppz, __ldg(D.tab[1][2][0] + gk), __ldg(D.tab[1][2][1] + gk), __ldg(D.tab[1][2][2] + gk));
-        st4(O.psi[1][2][szp] + pozp, ppz);
-      }
-      V4 p4;
-#pragma unroll
-      for (int e = 0; e < 4; ++e) p4.v[e] = upd(q0.v[e], kc4.v[e], __fadd_rn(__fadd_rn(dxp.v[e], dyp.v[e]), dzp.v[e]));
-      if (active) st4(O.f[0] + goff, p4);
-      goff += D.plane;
-      ++eit;
+  for (int n = 0; n < 7; ++n) q[n] = q[n + 1];
+  q[7] = v;
+}
+
+// vz_new[kz] from the p ring (logical order a[0..7] = p_old[kz-3 .. kz+4]), CPML in the z slabs, store if owned.
+__device__ __forceinline__ V4 fused_vz(const DomainView& D, const OutSet& O, const MainConst& K, MainCtx& C, const V4& a0, const V4& a1,
+                                       const V4& a2, const V4& a3, const V4& a4, const V4& a5, const V4& a6, const V4& a7, V4 vz4, int kz) {
+  V4 dzv = diff_8(a4, a3, a5, a2, a6, a1, a7, a0);
+  const int gk = kz + D.oz;
+  const bool inz = kz >= 0 && kz < D.nz;
+  if (inz && (kz < K.zl || kz >= K.zh)) {                      // block-uniform: this plane lies in a z slab
+    const int sz = kz < K.zl ? 0 : 1;
+    const long long poz = (long long)(kz - D.ls[2][sz]) * D.plane + K.zrow;
+    const float ta = __ldg(D.tab[0][2][0] + gk), tb = __ldg(D.tab[0][2][1] + gk), tk = __ldg(D.tab[0][2][2] + gk);
+    V4 psz = K.active ? ldg4(D.psi[0][2][sz] + poz) : zero4();
+    cpml4s(dzv, psz, ta, tb, tk);
+    if (K.active && kz >= K.z0 && kz < K.z1) st4(O.psi[0][2][sz] + poz, psz);     // lead-in / tail planes belong to another item
+  }
+  const float Bz = (!inz || gk == D.gn[2] - 1) ? 0.f : K.Bxy;
+  vz4 = upd4(vz4, Bz, Bz, Bz, dzv);
+  if (K.active && kz >= K.z0 && kz < K.z1) st4(C.gvz, vz4);
+  C.gvz += D.plane;
+  return vz4;
+}
+
+// One steady-state iteration: output plane k (m = k+7, kz = k+3).  R = rotation of the two rings on entry.
+template <int R, bool XY>
+__device__ __forceinline__ void fused_steady(const DomainView& D, const OutSet& O, const float* smem, float* ebuf, const FusedBars& Q,
+                                             const MainConst& K, MainCtx& C, int k) {
+#define PQ(n) C.pq[(R + 1 + (n)) & 7]
+#define WQ(n) C.wq[(R + 1 + (n)) & 7]
+  static_assert(R == 7, "canonical ring order: the rings are shifted, not renamed (an 8x unrolled body thrashes the 32 KB I-cache)");
+  const unsigned slot = C.it % FNS;
+  const float* st = smem + slot * F_STAGE_FLOATS;
+  // psi of plane k arrived during the previous iteration; start the loads of plane k+1 now
+  V4 psx, psy, ppx, ppy;
+  if (XY) {
+    psx = C.nvx; psy = C.nvy; ppx = C.npx; ppy = C.npy;
+    if (k + 1 < K.z1) {
+      if (K.sx >= 0) { C.nvx = ldg4(D.psi[0][0][K.sx] + C.pox + K.stride_px); C.npx = ldg4(D.psi[1][0][K.sx] + C.pox + K.stride_px); }
+      if (K.sy >= 0) { C.nvy = ldg4(D.psi[0][1][K.sy] + C.poy + K.stride_py); C.npy = ldg4(D.psi[1][1][K.sy] + C.poy + K.stride_py); }
     }
   }
+  mbar_wait(&Q.full[slot], (C.it / FNS) & 1);
+  shift_push(C.pq, ld4(st + F_OFF_PT + K.toff));                // newest p_old plane: PQ(7)
+  const float* row = st + K.boff;
+  const V4 c = ld4(row);
+  V4 dxv = diff_x<true>(ld4(row - 4), c, ld4(row + 4));
+  V4 dyv = diff_8(ld4(row + BW), c, ld4(row + 2 * BW), ld4(row - BW), ld4(row + 3 * BW), ld4(row - 2 * BW), ld4(row + 4 * BW),
+                  ld4(row - 3 * BW));
+  V4 vx4 = ld4(st + F_OFF_VX + K.exo);
+  V4 vy4 = ld4(st + F_OFF_VY + (K.ty + 4) * TX + 4 * K.tx);
+  V4 vz4 = ld4(st + F_OFF_VZ + K.toff);
+  const V4 kc4 = K.has_kc ? ld4(st + F_OFF_KC + K.toff) : splat4(D.kc0);
+  warp_arrive(&Q.empty[slot]);
+
+  // ---- velocity sub-update at plane k
+  if (XY) {
+    if (K.sx >= 0) {
+      cpml4(dxv, psx, ldg4(D.tab[0][0][0] + K.gi), ldg4(D.tab[0][0][1] + K.gi), ldg4(D.tab[0][0][2] + K.gi));
+      st4(O.psi[0][0][K.sx] + C.pox, psx);
+    }
+    if (K.sy >= 0) {
+      cpml4s(dyv, psy, __ldg(D.tab[0][1][0] + K.gj), __ldg(D.tab[0][1][1] + K.gj), __ldg(D.tab[0][1][2] + K.gj));
+      st4(O.psi[0][1][K.sy] + C.poy, psy);
+    }
+  }
+  vx4 = upd4(vx4, K.Bxy, K.Bxy, K.Bx3, dxv);
+  vy4 = upd4(vy4, K.By, K.By, K.By, dyv);
+  if (K.active) { st4(C.gvx, vx4); st4(C.gvy, vy4); }
+  const unsigned eb = C.eit & 1;
+  float* E = ebuf + eb * E_FLOATS;
+  // every main warp has passed the efull wait of the previous plane, so nobody still reads this buffer (see step_fused)
+  st4(E + K.exo, vx4);
+  st4(E + K.eyo, vy4);
+  warp_arrive(&Q.efull[eb]);
+
+  // ---- vz_new at kz+1/2 from p_old[kz-3 .. kz+4], then D-_z of the new vz ring
+  vz4 = fused_vz(D, O, K, C, PQ(0), PQ(1), PQ(2), PQ(3), PQ(4), PQ(5), PQ(6), PQ(7), vz4, k + 3);
+  shift_push(C.wq, vz4);                                         // WQ(7) = vz_new[k+3]
+  V4 dzp = diff_8(WQ(4), WQ(3), WQ(5), WQ(2), WQ(6), WQ(1), WQ(7), WQ(0));
+  V4 ppz;
+  const bool pz = k < K.zl || k >= K.zh;                         // block-uniform: plane k lies in a z slab
+  const int szp = k < K.zl ? 0 : 1;
+  const long long pozp = (long long)(k - D.ls[2][szp]) * D.plane + K.zrow;
+  if (pz) ppz = K.active ? ldg4(D.psi[1][2][szp] + pozp) : zero4();
+
+  // ---- pressure sub-update at plane k
+  mbar_wait(&Q.efull[eb], (C.eit >> 1) & 1);
+  const float* xr = E + K.exo;
+  V4 dxp = diff_x<false>(ld4(xr - 4), vx4, ld4(xr + 4));
+  const float* col = E + E_OFF_VY + K.ty * TX + 4 * K.tx;         // row ty of E.vy <-> y = j-4
+  V4 dyp = diff_8(vy4, ld4(col + 3 * TX), ld4(col + 5 * TX), ld4(col + 2 * TX), ld4(col + 6 * TX), ld4(col + TX), ld4(col + 7 * TX),
+                  ld4(col));
+  if (XY) {
+    if (K.sx >= 0) {
+      cpml4(dxp, ppx, ldg4(D.tab[1][0][0] + K.gi), ldg4(D.tab[1][0][1] + K.gi), ldg4(D.tab[1][0][2] + K.gi));
+      st4(O.psi[1][0][K.sx] + C.pox, ppx);
+      C.pox += K.stride_px;
+    }
+    if (K.sy >= 0) {
+      cpml4s(dyp, ppy, __ldg(D.tab[1][1][0] + K.gj), __ldg(D.tab[1][1][1] + K.gj), __ldg(D.tab[1][1][2] + K.gj));
+      st4(O.psi[1][1][K.sy] + C.poy, ppy);
+      C.poy += K.stride_py;
+    }
+  }
+  if (pz) {
+    const int gk = k + D.oz;
+    cpml4s(dzp, ppz, __ldg(D.tab[1][2][0] + gk), __ldg(D.tab[1][2][1] + gk), __ldg(D.tab[1][2][2] + gk));
+    if (K.active) st4(O.psi[1][2][szp] + pozp, ppz);
+  }
+  const float2 s0 = __fadd2_rn(__fadd2_rn(lo2(dxp), lo2(dyp)), lo2(dzp)), s1 = __fadd2_rn(__fadd2_rn(hi2(dxp), hi2(dyp)), hi2(dzp));
+  const V4 p4 = join2(__ffma2_rn(pk(-kc4.v[0], -kc4.v[1]), s0, lo2(PQ(0))), __ffma2_rn(pk(-kc4.v[2], -kc4.v[3]), s1, hi2(PQ(0))));
+  if (K.active) st4(C.gp, p4);
+  C.gvx += D.plane; C.gvy += D.plane; C.gp += D.plane;
+  ++C.it; ++C.eit;
+#undef PQ
+#undef WQ
+}
+
+template <bool XY>
+__device__ __forceinline__ void fused_main_item(const DomainView& D, const OutSet& O, const float* smem, float* ebuf, const FusedBars& Q,
+                                                const MainConst& K, MainCtx& C) {
+  const int z0 = K.z0, z1 = K.z1;
+#pragma unroll
+  for (int n = 0; n < 8; ++n) { C.pq[n] = zero4(); C.wq[n] = zero4(); }
+  // lead-in 1: planes z0-7 .. z0-1 of p_old only fill the ring
+  for (int m = z0 - 7; m < z0; ++m, ++C.it) {
+    const unsigned slot = C.it % FNS;
+    mbar_wait(&Q.full[slot], (C.it / FNS) & 1);
+    const V4 v = ld4(smem + slot * F_STAGE_FLOATS + F_OFF_PT + K.toff);
+    warp_arrive(&Q.empty[slot]);
+    shift_push(C.pq, v);
+  }
+  // lead-in 2: planes z0 .. z0+6 also produce vz_new[z0-4 .. z0+2]
+  for (int m = z0; m < z0 + 7; ++m, ++C.it) {
+    const unsigned slot = C.it % FNS;
+    const float* st = smem + slot * F_STAGE_FLOATS;
+    mbar_wait(&Q.full[slot], (C.it / FNS) & 1);
+    const V4 v = ld4(st + F_OFF_PT + K.toff);
+    V4 vz4 = ld4(st + F_OFF_VZ + K.toff);
+    warp_arrive(&Q.empty[slot]);
+    shift_push(C.pq, v);
+    vz4 = fused_vz(D, O, K, C, C.pq[0], C.pq[1], C.pq[2], C.pq[3], C.pq[4], C.pq[5], C.pq[6], C.pq[7], vz4, m - 4);
+    shift_push(C.wq, vz4);
+  }
+  // after lead-in 2 the rings are canonical for m = z0+6; one more rotation step puts the oldest entry at index 0 = R
+  if (XY) {
+    if (K.sx >= 0) { C.nvx = ldg4(D.psi[0][0][K.sx] + C.pox); C.npx = ldg4(D.psi[1][0][K.sx] + C.pox); }
+    if (K.sy >= 0) { C.nvy = ldg4(D.psi[0][1][K.sy] + C.poy); C.npy = ldg4(D.psi[1][1][K.sy] + C.poy); }
+  }
+  for (int k = z0; k < z1; ++k) fused_steady<7, XY>(D, O, smem, ebuf, Q, K, C, k);
+}
+
+__device__ __forceinline__ void fused_main(const DomainView& D, const OutSet& O, const float* smem, float* ebuf, const FusedBars& Q,
+                                           unsigned& it, unsigned& eit, int x0, int y0, int z0, int z1) {
+  const int tid = threadIdx.x;
+  MainConst K;
+  K.tx = tid & 15; K.ty = tid >> 4;
+  K.i = x0 + 4 * K.tx; K.j = y0 + K.ty;
+  K.z0 = z0; K.z1 = z1;
+  K.has_kc = D.kc != nullptr;
+  K.active = (K.i < D.nx) && (K.j < D.ny);
+  K.Bxy = K.active ? D.b0 : 0.f;
+  K.Bx3 = (K.i + 3 + D.ox) == D.gn[0] - 1 ? 0.f : K.Bxy;           // pinned last half node (R3)
+  K.By = (K.j + D.oy) == D.gn[1] - 1 ? 0.f : K.Bxy;
+  K.zrow = (long long)K.j * D.pitch + K.i;
+  K.boff = (K.ty + 7) * BW + 4 * K.tx + 8;                          // own float4 in the p box
+  K.toff = K.ty * TX + 4 * K.tx;                                    // own float4 in a plain tile
+  K.exo = K.ty * HW + 4 * K.tx + 4;                                 // own float4 in E.vx and in the vx x-halo tile
+  K.eyo = E_OFF_VY + (K.ty + 4) * TX + 4 * K.tx;                    // own float4 in E.vy
+  K.zl = D.ln[2][0];                                                // low z slab = local planes [0, zl)
+  K.zh = D.ln[2][1] > 0 ? D.ls[2][1] : 0x7fffffff;                  // high z slab = local planes [zh, nz)
+  const bool any_xy = touches(D, 0, x0, x0 + TX) || touches(D, 1, y0, y0 + TY);
+  K.sx = (any_xy && K.active) ? slab_side(D, 0, K.i) : -1;
+  K.sy = (any_xy && K.active) ? slab_side(D, 1, K.j) : -1;
+  K.stride_px = K.sx >= 0 ? (long long)D.ny * D.ln[0][K.sx] : 0;
+  K.stride_py = K.sy >= 0 ? (long long)D.ln[1][K.sy] * D.pitch : 0;
+  K.gi = K.i + D.ox; K.gj = K.j + D.oy;
+  MainCtx C;
+  C.it = it; C.eit = eit;
+  C.pox = K.sx >= 0 ? psi_index(D, 0, K.sx, K.i, K.j, z0) : 0;
+  C.poy = K.sy >= 0 ? psi_index(D, 1, K.sy, K.i, K.j, z0) : 0;
+  const long long goff = K.zrow + (long long)z0 * D.plane;
+  C.gvx = O.f[1] + goff; C.gvy = O.f[2] + goff; C.gp = O.f[0] + goff;
+  C.gvz = O.f[3] + K.zrow + (long long)(z0 - 4) * D.plane;          // first vz plane computed is z0-4 (stored from z0 on)
+  if (any_xy) fused_main_item<true>(D, O, smem, ebuf, Q, K, C);
+  else fused_main_item<false>(D, O, smem, ebuf, Q, K, C);
+  it = C.it; eit = C.eit;
 }
 
 // ---- halo warps: the redundantly computed ghost of the tile, never stored to global memory ----------------
@@ -302,19 +367,19 @@ __device__ __forceinline__ void fused_halo(const TMaps& tm, const DomainView& D,
         cpml4s(dyv, psy, __ldg(D.tab[0][1][0] + gj), __ldg(D.tab[0][1][1] + gj), __ldg(D.tab[0][1][2] + gj));
         poy += stride_py;
       }
-#pragma unroll
-      for (int e = 0; e < 4; ++e) vy4.v[e] = upd(vy4.v[e], By, dyv.v[e]);
+      vy4 = upd4(vy4, By, By, By, dyv);
       if (do_x) {
         if (sx >= 0) {
           cpml4(dxv, psx, ldg4(D.tab[0][0][0] + gi), ldg4(D.tab[0][0][1] + gi), ldg4(D.tab[0][0][2] + gi));
           pox += stride_px;
         }
-        vx4.v[0] = upd(vx4.v[0], Bvx, dxv.v[0]); vx4.v[1] = upd(vx4.v[1], Bvx, dxv.v[1]);
-        vx4.v[2] = upd(vx4.v[2], Bvx, dxv.v[2]); vx4.v[3] = upd(vx4.v[3], Bx3, dxv.v[3]);
+        vx4 = upd4(vx4, Bvx, Bvx, Bx3, dxv);
       }
-      const unsigned eb = eit & 1, eu = eit >> 1;
+      const unsigned eb = eit & 1;
       float* E = ebuf + eb * E_FLOATS;
-      mbar_wait(&Q.eempty[eb], (eu & 1) ^ 1);
+      // this buffer was last read for plane eit-2; every main warp is past that once the previous plane's efull phase
+      // is complete (a main warp arrives there only after it has finished reading the plane before)
+      if (eit > 0) mbar_wait(&Q.efull[eb ^ 1], ((eit - 1) >> 1) & 1);
       st4(E + E_OFF_VY + eyo, vy4);
       if (do_x) st4(E + exo, vx4);
       warp_arrive(&Q.efull[eb]);
@@ -328,14 +393,13 @@ __global__ void __launch_bounds__(FNT, 1) step_fused(const __grid_constant__ TMa
   extern __shared__ __align__(128) unsigned char smem_raw[];
   float* smem = reinterpret_cast<float*>(smem_raw);
   float* ebuf = smem + FNS * F_STAGE_FLOATS;
-  __shared__ __align__(8) uint64_t bars[2 * FNS + 4];
+  __shared__ __align__(8) uint64_t bars[2 * FNS + 2];
   __shared__ int s_item;
-  const FusedBars Q{bars, bars + FNS, bars + 2 * FNS, bars + 2 * FNS + 2};
+  const FusedBars Q{bars, bars + FNS, bars + 2 * FNS};
   if (threadIdx.x == 0) {
 #pragma unroll
     for (int s = 0; s < FNS; ++s) { mbar_init(&Q.full[s], 1); mbar_init(&Q.empty[s], FNW); }
     mbar_init(&Q.efull[0], FNW); mbar_init(&Q.efull[1], FNW);
-    mbar_init(&Q.eempty[0], FW_MAIN); mbar_init(&Q.eempty[1], FW_MAIN);
     fence_barrier_init();
     if (blockIdx.x == 0) *S.other = 0u;
   }
@@ -346,11 +410,7 @@ __global__ void __launch_bounds__(FNT, 1) step_fused(const __grid_constant__ TMa
   // warpgroups take the registers the halo warpgroup gives up (3 warps per SM sub-partition: 2 x 216 + 72 <= 512).
   if (warp < FW_MAIN) {
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(F_REGS_MAIN));
-    while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) {
-      fused_main(D, O, smem, ebuf, Q, it, eit, x0, y0, z0, z1);
-      it += z1 - z0 + 14;
-      eit += z1 - z0;
-    }
+    while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) fused_main(D, O, smem, ebuf, Q, it, eit, x0, y0, z0, z1);
   } else {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(F_REGS_HALO));
     const bool has_kc = D.kc != nullptr;

@@ -234,20 +234,38 @@ __device__ __forceinline__ V4 diff_x(const V4& l, const V4& c, const V4& r) {
   }
   return d;
 }
+// Packed fp32x2 forms (sm_100a FADD2 / FMUL2 / FFMA2: two independent IEEE operations per instruction, so the bits
+// are those of the scalar sequence; they halve the issue slots of the arithmetic).
+__device__ __forceinline__ float2 pk(float a, float b) { return make_float2(a, b); }
+__device__ __forceinline__ float2 sub2(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
+__device__ __forceinline__ float2 stag_diff2(float2 h1, float2 l1, float2 h2, float2 l2, float2 h3, float2 l3, float2 h4, float2 l4) {
+  float2 d = __fmul2_rn(pk(FDTD_C1, FDTD_C1), sub2(h1, l1));
+  d = __ffma2_rn(pk(FDTD_C2, FDTD_C2), sub2(h2, l2), d);
+  d = __ffma2_rn(pk(FDTD_C3, FDTD_C3), sub2(h3, l3), d);
+  d = __ffma2_rn(pk(FDTD_C4, FDTD_C4), sub2(h4, l4), d);
+  return d;
+}
+__device__ __forceinline__ float2 lo2(const V4& a) { return make_float2(a.v[0], a.v[1]); }
+__device__ __forceinline__ float2 hi2(const V4& a) { return make_float2(a.v[2], a.v[3]); }
+__device__ __forceinline__ V4 join2(float2 a, float2 b) { V4 r; r.v[0] = a.x; r.v[1] = a.y; r.v[2] = b.x; r.v[3] = b.y; return r; }
 __device__ __forceinline__ V4 diff_8(const V4& h1, const V4& l1, const V4& h2, const V4& l2, const V4& h3, const V4& l3, const V4& h4,
                                      const V4& l4) {
-  V4 d;
-#pragma unroll
-  for (int e = 0; e < 4; ++e) d.v[e] = stag_diff(h1.v[e], l1.v[e], h2.v[e], l2.v[e], h3.v[e], l3.v[e], h4.v[e], l4.v[e]);
-  return d;
+  return join2(stag_diff2(lo2(h1), lo2(l1), lo2(h2), lo2(l2), lo2(h3), lo2(l3), lo2(h4), lo2(l4)),
+               stag_diff2(hi2(h1), hi2(l1), hi2(h2), hi2(l2), hi2(h3), hi2(l3), hi2(h4), hi2(l4)));
+}
+// f - coef d for four points, coefficients (c01, c01, c2, c3)
+__device__ __forceinline__ V4 upd4(const V4& f, float c01, float c2, float c3, const V4& d) {
+  return join2(__ffma2_rn(pk(-c01, -c01), lo2(d), lo2(f)), __ffma2_rn(pk(-c2, -c3), hi2(d), hi2(f)));
 }
 __device__ __forceinline__ void cpml4(V4& d, V4& ps, const V4& a, const V4& b, const V4& ik) {
 #pragma unroll
   for (int e = 0; e < 4; ++e) d.v[e] = cpml_apply(d.v[e], ps.v[e], a.v[e], b.v[e], ik.v[e]);
 }
 __device__ __forceinline__ void cpml4s(V4& d, V4& ps, float a, float b, float ik) {
-#pragma unroll
-  for (int e = 0; e < 4; ++e) d.v[e] = cpml_apply(d.v[e], ps.v[e], a, b, ik);
+  const float2 a2 = pk(a, a), b2 = pk(b, b), k2 = pk(ik, ik);
+  const float2 p0 = __ffma2_rn(b2, lo2(ps), __fmul2_rn(a2, lo2(d))), p1 = __ffma2_rn(b2, hi2(ps), __fmul2_rn(a2, hi2(d)));
+  d = join2(__ffma2_rn(lo2(d), k2, p0), __ffma2_rn(hi2(d), k2, p1));
+  ps = join2(p0, p1);
 }
 
 // ring bookkeeping shared by both kernels
