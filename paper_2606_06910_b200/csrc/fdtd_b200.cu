@@ -293,7 +293,7 @@ void plan_items_fused(Domain& d, int grid) {
   S.ntx = (v.nx + TX - 1) / TX;
   S.nty = (v.ny + TY - 1) / TY;
   const long long tiles = (long long)S.ntx * S.nty;
-  long long zc = (long long)v.nz * tiles / (6LL * std::max(grid, 1));
+  long long zc = (long long)v.nz * tiles / (12LL * std::max(grid, 1));
   zc = std::max(32LL, std::min(256LL, zc));
   if (const char* e = getenv("FDTD_ZCHUNK_FUSED")) zc = std::max(1, atoi(e));
   int n = (int)((v.nz + zc - 1) / zc);
