@@ -33,8 +33,10 @@ def parse():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config3", choices=["config1", "config2", "config3", "config4"])
-    ap.add_argument("--kernel", default="fused", choices=["fused", "two-pass"],
-                    help="fused: one single-pass launch per step (FDTD_KERNEL_FUSED, 32 B/pt); two-pass: update_v + update_p (48 B/pt)")
+    ap.add_argument("--kernel", default="two-pass", choices=["fused", "two-pass"],
+                    help="two-pass: update_v + update_p (48 B/pt, the default); fused: one single-pass launch per step "
+                         "(FDTD_KERNEL_FUSED, 32 B/pt, twice the field memory)")
+    ap.add_argument("--no-alt", action="store_true", help="do not also time the other kernel for the 'alt_kernel' entry")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpml-off", action="store_true", help="same total grid with plain walls (CPML overhead run, P:228)")
@@ -250,27 +252,39 @@ def main():
 
     fused = args.kernel == "fused"
     kern = binding.FDTD_KERNEL_FUSED if fused else binding.FDTD_KERNEL_AUTO
-    sim = binding.from_workload(w, device=local, kernel=kern)
-    for f in range(1, 4):                       # non-trivial state everywhere (values do not change the traffic)
-        sim.fill_hash(f, 99, 1e-3)
-    sim.step(W)
-    barrier()
-    sampler = ClockSampler(local) if rank == 0 else None
-    l0 = sim.launch_count()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    sim.step(K)
-    e1.record()
-    barrier()
-    ms = e0.elapsed_time(e1)
-    launches = sim.launch_count() - l0
-    # per-kernel durations, CUDA events on the launching stream, same K steps of the same state
-    prof = sim.step_profiled(K)
-    clocks = sampler.stop() if sampler else None
-    ms = max_over_ranks(ms, world, "cuda")
-    sim.destroy()
-    del sim
-    torch.cuda.empty_cache()
+
+    def timed_run(kernel, sample_clocks):
+        """W warm-up steps, then K steps between two CUDA events (barrier + synchronize on both sides), then the same
+        K steps again with an event after every launch group for the per-kernel split."""
+        sim = binding.from_workload(w, device=local, kernel=kernel)
+        for f in range(1, 4):                   # non-trivial state everywhere (values do not change the traffic)
+            sim.fill_hash(f, 99, 1e-3)
+        sim.step(W)
+        barrier()
+        sampler = ClockSampler(local) if (rank == 0 and sample_clocks) else None
+        l0 = sim.launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        sim.step(K)
+        e1.record()
+        barrier()
+        t = e0.elapsed_time(e1)
+        n_launch = sim.launch_count() - l0
+        split = sim.step_profiled(K)
+        clk = sampler.stop() if sampler else None
+        t = max_over_ranks(t, world, "cuda")
+        sim.destroy()
+        del sim
+        torch.cuda.empty_cache()
+        return t, n_launch, split, clk
+
+    ms, launches, prof, clocks = timed_run(kern, True)
+    alt = None
+    if not args.no_alt and w.total[0] % 4 == 0:
+        other = binding.FDTD_KERNEL_AUTO if fused else binding.FDTD_KERNEL_FUSED
+        a_ms, _, a_prof, _ = timed_run(other, False)
+        alt = {"kernel": "two-pass" if fused else "fused", "value": throughput_mpts(w.points, K, world, a_ms * 1e-3), "unit": UNIT,
+               "ms_per_step": a_ms / K, "kernels_ms_per_step": {k: v / K for k, v in a_prof.items() if v > 0}}
 
     # ---- end to end through the C ABI with host buffers: model up, K steps, pressure field down
     e2e = None
@@ -327,8 +341,11 @@ def main():
         "config": {"workload": w.name + ("-cpml-off" if args.cpml_off else ""), "total_grid": list(w.total), "cpml": list(w.cpml),
                    "medium": "heterogeneous c (Kc array)" if w.c is not None else "homogeneous", "sources": int(w.sources.shape[0]),
                    "kernel": args.kernel, "parallelism": "replicas x%d" % world, "l2": "inputs larger than L2 (fields %.1f GB)" % (w.points * 16 / 1e9)},
-        "roofline": roof, "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e,
+        "roofline": roof, "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e, "alt_kernel": alt,
     }
+    if alt is not None:
+        ab = (bv + bp) if fused else bf                # algorithmic bytes of the other kernel structure
+        alt["step_frac_of_peak"] = ab / (alt["ms_per_step"] * 1e-3) / 1e9 / peak
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = oracle_sample(w, 24)
     print(json.dumps(line))

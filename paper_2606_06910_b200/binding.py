@@ -223,6 +223,11 @@ class Fdtd:
         if getattr(self, "_h", None):
             rc = lib.fdtd_destroy(self._h)
             self._h = None
+            big = self.workspace_bytes > (1 << 30)
+            self._ws = None                      # the context is gone: give the workspace back
+            if big:                              # ... to the driver too, so the next large context is one contiguous block
+                import torch
+                torch.cuda.empty_cache()
             _check(rc, "fdtd_destroy")
 
     close = destroy

@@ -82,9 +82,20 @@ def test_config2_full_size_windows(B):
     sim.destroy()
 
 
-def test_config3_full_size_windows_heterogeneous(B):
+@pytest.mark.parametrize("kernel", [0, 2])
+def test_config3_full_size_windows_heterogeneous(B, kernel):
     w = inputs.config(3, steps=8)
-    sim = B.from_workload(w)
+    sim = B.from_workload(w, kernel=kernel)
+    _check(B, w, sim)
+    sim.destroy()
+
+
+def test_config4_full_size_windows_fused_step(B):
+    """The single-pass step at 1600^3: two copies of the state (131 GB of fields + psi) in one workspace, 64-bit offsets in
+    both, odd number of buffer swaps."""
+    w = inputs.config(4, steps=8)
+    sim = B.from_workload(w, kernel=B.FDTD_KERNEL_FUSED)
+    assert sim.workspace_bytes > 130e9
     _check(B, w, sim)
     sim.destroy()
 
