@@ -152,6 +152,34 @@ def test_fused_and_two_pass_agree_bitwise(B, shape, cpml, het):
         assert np.array_equal(a.view(np.uint32), b.view(np.uint32)), n
 
 
+@pytest.mark.parametrize("kernel", [1, 0, 2])
+def test_paper_cpml_parameter_set_parity(B, kernel):
+    """the paper's own CPML set (Table 2): q = 3, R = 1e-8, kappa_max = 5 (the 1/kappa
+    tables are no longer 1), alpha_max = 0.05 sigma_max, L = 20; random state, source inside the layer, 40 steps."""
+    L = 20
+    smax = -4.0 * math.log(1e-8) / (2.0 * L * 1.0)
+    kw = dict(dt=0.4, cpml_order=3, cpml_R0=1e-8, cpml_kappa_max=5.0, cpml_alpha_max=0.05 * smax, cpml_c_ref=1.0)
+    shape, cpml = (24, 28, 32), (L,) * 6
+    sim = B.Fdtd(shape, cpml, kernel=kernel, **kw)
+    o = Oracle(shape, cpml, **kw)
+    a, b, ik = sim.cpml_table(0, 1)
+    assert ik.min() < 0.25 and np.array_equal(ik, o.cpml_table(0, 1)[2])            # kappa really is stretched
+    src = np.array([[32, 34, 36], [7, 30, 60]], np.int32)
+    wav = np.stack([inputs.ricker(40, 0.4, t0=5.0), 0.05 * np.ones(40, np.float32)])
+    for s_ in (sim, o):
+        s_.set_sources(src, wav)
+    for f in range(4):
+        sim.fill_hash(f, 9, 0.5)
+        o.fill_hash(f, 9, scale=0.5)
+    sim.step(40)
+    o.step(40)
+    for f in range(4):
+        assert rel(sim.get_field(f), o.get(f)) <= TOL, (f, rel(sim.get_field(f), o.get(f)))
+    for q in range(6):
+        assert rel(sim.get_psi(q), o.get(4 + q)) <= TOL, q
+    sim.destroy()
+
+
 def test_periodic_dispersion_on_gpu(B):
     """Pin P2 on the CUDA path (reference kernel, periodic): p^{n+1} + p^{n-1} = (2 - 4S) p^n."""
     N, mode = 16, (1, 2, 3)
