@@ -161,6 +161,8 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, u
       "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
       : "memory");
 }
+// non-binding prefetch of one 128-B line into L2 (psi of a later plane: streamed once, so only latency matters)
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
@@ -177,6 +179,7 @@ constexpr int TY = 16;             // tile height in y (rows)
 constexpr int NT = 256;            // threads per CTA
 constexpr int NW = NT / 32;        // warps per CTA
 constexpr int NS = 4;              // ring stages
+constexpr int PSI_AHEAD = 3;       // planes of psi prefetched into L2 ahead of their use in the x / y slabs
 constexpr int HW = TX + 8;         // x-halo tile width: columns x0-4 .. x0+TX+3
 constexpr int VH = TY + 7;         // p rows for update_v: y0-3 .. y0+TY+3
 constexpr int PH = TY + 8;         // vy rows for update_p: y0-4 .. y0+TY+3
@@ -346,8 +349,8 @@ __device__ __forceinline__ void v_item(const TMaps& tm, const DomainView& D, flo
     V4 psx, psy, psz;
     const int sz = zz ? slab_side(D, 2, kz) : -1;
     float* ppz = nullptr;
-    if (xy && sx >= 0) psx = ld4(ppx);
-    if (xy && sy >= 0) psy = ld4(ppy);
+    if (xy && sx >= 0) { psx = ld4(ppx); prefetch_l2(ppx + PSI_AHEAD * stride_px); }
+    if (xy && sy >= 0) { psy = ld4(ppy); prefetch_l2(ppy + PSI_AHEAD * stride_py); }
     if (sz >= 0 && active) { ppz = D.psi[0][2][sz] + psi_index(D, 2, sz, i, j, kz); psz = ld4(ppz); }
     // producer duty: refill the stage every warp released in the previous iteration
     if (tid == 0 && m > m_begin && (m - 1 + NS) < m_end) {
@@ -502,8 +505,8 @@ __device__ __forceinline__ void p_item(const TMaps& tm, const DomainView& D, flo
     V4 psx, psy, psz;
     const int sz = out ? slab_side(D, 2, k) : -1;
     float* ppz = nullptr;
-    if (out && sx >= 0) psx = ld4(ppx);
-    if (out && sy >= 0) psy = ld4(ppy);
+    if (out && sx >= 0) { psx = ld4(ppx); prefetch_l2(ppx + PSI_AHEAD * stride_px); }
+    if (out && sy >= 0) { psy = ld4(ppy); prefetch_l2(ppy + PSI_AHEAD * stride_py); }
     if (sz >= 0 && active) { ppz = D.psi[1][2][sz] + psi_index(D, 2, sz, i, j, k); psz = ld4(ppz); }
     if (tid == 0 && m > m_begin && (m - 1 + NS) < m_end) {
       const unsigned ps = (it - 1) % NS;
