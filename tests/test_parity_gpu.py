@@ -180,6 +180,35 @@ def test_paper_cpml_parameter_set_parity(B, kernel):
     sim.destroy()
 
 
+@pytest.mark.parametrize("kernel", [1, 0, 2])
+@pytest.mark.parametrize("shape,cpml", [
+    ((8, 3, 2), (0,) * 6),                      # thinner than the stencil radius in y and z, far smaller than one tile
+    ((4, 1, 1), (0,) * 6),                      # a single row of four points: every read but three is outside the grid
+    ((4, 5, 3), (2, 2, 1, 1, 1, 1)),            # layers that meet in the middle: every point is in some layer
+    ((12, 4, 40), (0, 0, 0, 0, 3, 3)),          # a thin column through several z planes
+])
+def test_degenerate_grids_parity(B, kernel, shape, cpml):
+    """Edge cases: grids below the tile and below the stencil reach, layers covering the whole grid, no sources,
+    zero steps.  All three CUDA paths against the oracle."""
+    kw = dict(dt=0.35, cpml_alpha_max=math.pi * inputs.F0)
+    sim = B.Fdtd(shape, cpml, kernel=kernel, **kw)
+    o = Oracle(shape, cpml, **kw)
+    for f in range(4):
+        sim.fill_hash(f, 21, 0.5)
+        o.fill_hash(f, 21, scale=0.5)
+    before = [sim.get_field(f) for f in range(4)]
+    sim.step(0)                                                     # zero steps: nothing changes, nothing is launched
+    for f in range(4):
+        assert np.array_equal(sim.get_field(f), before[f])
+    sim.step(5)
+    o.step(5)
+    for f in range(4):
+        assert rel(sim.get_field(f), o.get(f)) <= TOL, (f, rel(sim.get_field(f), o.get(f)))
+    for q in range(6):
+        assert rel(sim.get_psi(q), o.get(4 + q)) <= TOL, q
+    sim.destroy()
+
+
 def test_periodic_dispersion_on_gpu(B):
     """Pin P2 on the CUDA path (reference kernel, periodic): p^{n+1} + p^{n-1} = (2 - 4S) p^n."""
     N, mode = 16, (1, 2, 3)
