@@ -32,12 +32,18 @@ enum {
   FDTD_EINVAL = -1,     /* bad size / parameter (dt <= 0, grid smaller than the layers, source out of range ...) */
   FDTD_EWORKSPACE = -2, /* workspace NULL, misaligned (256 B) or smaller than fdtd_workspace_bytes() */
   FDTD_ECUDA = -3,      /* a CUDA runtime / driver call failed; fdtd_last_error() has the text */
-  FDTD_EUNSUPPORTED = -4 /* valid per the paper but not built (e.g. heterogeneous density, R6 / NEXT-3) */
+  FDTD_EUNSUPPORTED = -4 /* valid per the paper but not built in this configuration (e.g. a density array with   */
+                         /* FDTD_KERNEL_FUSED, or without params.density = FDTD_DENSITY_ARRAY)                   */
 };
 
 enum { FDTD_P = 0, FDTD_VX = 1, FDTD_VY = 2, FDTD_VZ = 3 };                 /* field selectors */
 enum { FDTD_PSI_VX = 0, FDTD_PSI_VY = 1, FDTD_PSI_VZ = 2, FDTD_PSI_PX = 3, FDTD_PSI_PY = 4, FDTD_PSI_PZ = 5 };
 enum { FDTD_WALL = 0, FDTD_PERIODIC = 1 };
+enum {
+  FDTD_DENSITY_UNIFORM = 0, /* rho is one number: dt/(rho dx) is a scalar                                     */
+  FDTD_DENSITY_ARRAY = 1    /* the workspace also holds dt/(rho_bar dx) at the half nodes of vx, vy, vz (+12 B */
+                            /* per point), so fdtd_set_model accepts a heterogeneous rho (R6)     */
+};
 enum {
   FDTD_KERNEL_AUTO = 0, /* TMA-staged, z-streaming tile kernels (the product path)                        */
   FDTD_KERNEL_REF = 1,  /* one thread per point, global loads only; also the only path for FDTD_PERIODIC   */
@@ -64,6 +70,7 @@ typedef struct {
   int32_t ghost;          /* ghost depth g in cells on every internal interface                 */
   int32_t substeps_per_exchange; /* m sub-updates (v or p) between halo exchanges; needs g >= 4 m (R20)      */
   int32_t kernel;         /* FDTD_KERNEL_AUTO / FDTD_KERNEL_REF / FDTD_KERNEL_FUSED                          */
+  int32_t density;        /* FDTD_DENSITY_UNIFORM / FDTD_DENSITY_ARRAY (not with FDTD_KERNEL_FUSED)          */
   int32_t device;         /* CUDA device ordinal                                                             */
   void* stream;           /* cudaStream_t the work is enqueued on (0 = legacy default stream)                */
   void* workspace;        /* DEVICE memory, 256-byte aligned, owned by the caller, must outlive the context  */
@@ -82,9 +89,10 @@ uint64_t fdtd_workspace_bytes(const fdtd_params* params);
 fdtd_ctx* fdtd_create(const fdtd_params* params);
 
 /* Medium (R6): c and rho are HOST arrays of the total grid (Nz*Ny*Nx fp32, x fastest) or NULL for 1.0
- * everywhere.  The library forms K dt/dx = rho c^2 dt/dx per node and dt/(rho dx) (double arithmetic, rounded
- * once to fp32) and copies them to the device before returning (synchronises the stream).  A non-uniform rho
- * returns FDTD_EUNSUPPORTED. */
+ * everywhere.  The library forms K dt/dx = rho c^2 dt/dx per node and dt/(rho_bar dx) per half node, rho_bar = mean
+ * of the two adjacent nodes (the last node repeats itself), in double arithmetic rounded once to fp32, and copies
+ * them to the device before returning (synchronises the stream).  A non-uniform rho needs
+ * params.density = FDTD_DENSITY_ARRAY, else FDTD_EUNSUPPORTED. */
 int fdtd_set_model(fdtd_ctx* ctx, const float* c_host, const float* rho_host);
 
 /* Point sources injected into p (P:193 gives the Ricker shape; R14): after the pressure sub-update of step n,

@@ -16,6 +16,7 @@ FDTD_P, FDTD_VX, FDTD_VY, FDTD_VZ = 0, 1, 2, 3
 FDTD_PSI_VX, FDTD_PSI_VY, FDTD_PSI_VZ, FDTD_PSI_PX, FDTD_PSI_PY, FDTD_PSI_PZ = range(6)
 FDTD_WALL, FDTD_PERIODIC = 0, 1
 FDTD_KERNEL_AUTO, FDTD_KERNEL_REF, FDTD_KERNEL_FUSED = 0, 1, 2
+FDTD_DENSITY_UNIFORM, FDTD_DENSITY_ARRAY = 0, 1
 FDTD_OK, FDTD_EINVAL, FDTD_EWORKSPACE, FDTD_ECUDA, FDTD_EUNSUPPORTED = 0, -1, -2, -3, -4
 
 # every symbol include/fdtd_b200.h declares
@@ -42,6 +43,7 @@ class fdtd_params(C.Structure):
         ("ghost", C.c_int32),
         ("substeps_per_exchange", C.c_int32),
         ("kernel", C.c_int32),
+        ("density", C.c_int32),
         ("device", C.c_int32),
         ("stream", C.c_void_p),
         ("workspace", C.c_void_p),
@@ -103,7 +105,7 @@ def fdtd_coeffs():
 
 def make_params(n_interior, cpml=(0,) * 6, dx=1.0, dt=0.4, cpml_order=2, cpml_R0=1e-5, cpml_kappa_max=1.0,
                 cpml_alpha_max=0.0, cpml_c_ref=1.0, boundary=FDTD_WALL, decomp=(1, 1, 1), ghost=0, substeps=0,
-                kernel=FDTD_KERNEL_AUTO, device=0):
+                kernel=FDTD_KERNEL_AUTO, density=FDTD_DENSITY_UNIFORM, device=0):
     p = fdtd_params()
     p.n_interior[:] = [int(v) for v in n_interior]
     p.cpml[:] = [int(v) for v in cpml]
@@ -113,7 +115,7 @@ def make_params(n_interior, cpml=(0,) * 6, dx=1.0, dt=0.4, cpml_order=2, cpml_R0
     p.cpml_alpha_max, p.cpml_c_ref = float(cpml_alpha_max), float(cpml_c_ref)
     p.decomp[:] = [int(v) for v in decomp]
     p.ghost, p.substeps_per_exchange = int(ghost), int(substeps)
-    p.kernel, p.device = int(kernel), int(device)
+    p.kernel, p.density, p.device = int(kernel), int(density), int(device)
     return p
 
 

@@ -88,6 +88,9 @@ Geometry make_geometry(const fdtd_params& P) {
   if (P.kernel < FDTD_KERNEL_AUTO || P.kernel > FDTD_KERNEL_FUSED) return bad("unknown kernel selector");
   if (P.kernel == FDTD_KERNEL_FUSED && (P.boundary == FDTD_PERIODIC || (n_total_x(P) % 4) != 0))
     return bad("FDTD_KERNEL_FUSED needs WALL boundaries and a total Nx that is a multiple of 4");
+  if (P.density != FDTD_DENSITY_UNIFORM && P.density != FDTD_DENSITY_ARRAY) return bad("unknown density selector");
+  if (P.density == FDTD_DENSITY_ARRAY && P.kernel == FDTD_KERNEL_FUSED)
+    return bad("FDTD_KERNEL_FUSED is not built for a heterogeneous density (use FDTD_KERNEL_AUTO)");
   if (P.boundary == FDTD_PERIODIC)
     for (int f = 0; f < 6; ++f) if (P.cpml[f]) return bad("PERIODIC excludes CPML");
   for (int f = 0; f < 6; ++f)
@@ -140,6 +143,7 @@ struct Layout {
     int ls[3][2], ln[3][2];
     uint64_t f[4], kc, psi[2][3][2], src_off, counters;
     uint64_t f2[4], psi2[2][3][2];   // fused mode: second state
+    uint64_t bq[3];                  // FDTD_DENSITY_ARRAY: dt/(rho_bar dx) at the half nodes of vx, vy, vz
   };
   std::vector<Dom> doms;
   uint64_t tab[2][3][3];
@@ -193,6 +197,8 @@ Layout make_layout(const fdtd_params& P, const Geometry& G) {
             d.psi2[fam][2][s] = take((uint64_t)d.pitch * d.n[1] * d.ln[2][s] * 4 + 16);
           }
       }
+      if (P.density == FDTD_DENSITY_ARRAY)
+        for (int a = 0; a < 3; ++a) d.bq[a] = take(vol);
       d.src_off = take(MAX_SRC * sizeof(long long));
       d.counters = take(64);
       L.doms.push_back(d);
@@ -329,7 +335,8 @@ int launch_substep(fdtd_ctx* c, Domain& d, int which /*0 = v, 1 = p*/) {
     Sched S = d.sched;
     S.counter = d.counters + which;
     S.other = d.counters + (1 - which);
-    if (which == 0) update_v_tiled<<<std::min(c->grid_v, S.nitems), NT, V_SMEM_BYTES, c->stream>>>(d.tm, v, S);
+    if (which == 0 && v.bq[0]) update_v_tiled<true><<<std::min(c->grid_v, S.nitems), NT, V_SMEM_BYTES, c->stream>>>(d.tm, v, S);
+    else if (which == 0) update_v_tiled<false><<<std::min(c->grid_v, S.nitems), NT, V_SMEM_BYTES, c->stream>>>(d.tm, v, S);
     else update_p_tiled<<<std::min(c->grid_p, S.nitems), NT, P_SMEM_BYTES, c->stream>>>(d.tm, v, S);
   }
   c->launches++;
@@ -606,6 +613,7 @@ fdtd_ctx* fdtd_create(const fdtd_params* P) {
       v.periodic = P->boundary == FDTD_PERIODIC;
       for (int f = 0; f < 4; ++f) v.f[f] = (float*)(c->ws + ld.f[f]);
       v.kc = nullptr;
+      for (int a = 0; a < 3; ++a) v.bq[a] = nullptr;
       v.kc0 = (float)(1.0 * 1.0 * 1.0 * P->dt / P->dx);
       v.b0 = (float)(P->dt / (1.0 * P->dx));
       for (int a = 0; a < 3; ++a)
@@ -647,11 +655,13 @@ fdtd_ctx* fdtd_create(const fdtd_params* P) {
     }
 
   if (!c->use_ref) {
-    if ((e = cudaFuncSetAttribute(update_v_tiled, cudaFuncAttributeMaxDynamicSharedMemorySize, V_SMEM_BYTES)) != cudaSuccess)
+    if ((e = cudaFuncSetAttribute(update_v_tiled<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, V_SMEM_BYTES)) != cudaSuccess ||
+        (e = cudaFuncSetAttribute(update_v_tiled<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, V_SMEM_BYTES)) != cudaSuccess)
       return fail(c, e, "cudaFuncSetAttribute(update_v_tiled)");
     if ((e = cudaFuncSetAttribute(update_p_tiled, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM_BYTES)) != cudaSuccess)
       return fail(c, e, "cudaFuncSetAttribute(update_p_tiled)");
-    if (plan_launch(c, (const void*)update_v_tiled, V_SMEM_BYTES, &c->grid_v) ||
+    if (plan_launch(c, P->density == FDTD_DENSITY_ARRAY ? (const void*)update_v_tiled<true> : (const void*)update_v_tiled<false>,
+                    V_SMEM_BYTES, &c->grid_v) ||
         plan_launch(c, (const void*)update_p_tiled, P_SMEM_BYTES, &c->grid_p)) { delete c; return nullptr; }
     for (auto& d : c->doms) plan_items(d, std::min(c->grid_v, c->grid_p));
     if (c->fused) {
@@ -672,16 +682,66 @@ int fdtd_dims(const fdtd_ctx* c, int32_t out[3]) {
 
 int64_t fdtd_launch_count(const fdtd_ctx* c) { return c ? c->launches : -1; }
 
+// Heterogeneous density ("coefficients are absorbed"; reading R6): K dt/dx = rho c^2 dt/dx at the nodes and
+// dt/(rho_bar dx) at the half nodes of vx, vy, vz with rho_bar the mean of the two adjacent nodes (the last node of an
+// axis repeats itself; that half node is pinned anyway, R3).  Formed on the host in double from the fp32 inputs, rounded
+// once, then scattered to the domains (ghost cells included, so subdomains see the global neighbour).
+static int set_model_density_array(fdtd_ctx* c, const float* c_host, const float* rho_host) {
+  if (c->P.density != FDTD_DENSITY_ARRAY) {
+    set_err("a heterogeneous rho needs params.density = FDTD_DENSITY_ARRAY (the workspace must hold the three dt/(rho_bar dx) arrays)");
+    return FDTD_EUNSUPPORTED;
+  }
+  const long long nx = c->G.gn[0], ny = c->G.gn[1], nz = c->G.gn[2];
+  const size_t n = (size_t)nx * ny * nz;
+  const double dt = c->P.dt, dx = c->P.dx;
+  std::vector<float> kc(n), bq[3];
+  for (int a = 0; a < 3; ++a) bq[a].resize(n);
+  for (size_t q = 0; q < n; ++q) {
+    const double cc = c_host ? (double)c_host[q] : 1.0, rr = (double)rho_host[q];
+    if (!(rr > 0.0) || rr > 1e30 || !(cc > 0.0) || cc > 1e30) { set_err("c and rho must be positive and finite"); return FDTD_EINVAL; }
+    kc[q] = (float)(rr * cc * cc * dt / dx);
+  }
+  for (long long k = 0; k < nz; ++k)
+    for (long long j = 0; j < ny; ++j)
+      for (long long i = 0; i < nx; ++i) {
+        const size_t q = (size_t)((k * ny + j) * nx + i);
+        const double r0 = rho_host[q];
+        const double rx = rho_host[i + 1 < nx ? q + 1 : q], ry = rho_host[j + 1 < ny ? q + (size_t)nx : q],
+                     rz = rho_host[k + 1 < nz ? q + (size_t)(nx * ny) : q];
+        bq[0][q] = (float)(dt / (0.5 * (r0 + rx) * dx));
+        bq[1][q] = (float)(dt / (0.5 * (r0 + ry) * dx));
+        bq[2][q] = (float)(dt / (0.5 * (r0 + rz) * dx));
+      }
+  std::vector<float*> bases;
+  for (size_t k = 0; k < c->doms.size(); ++k) bases.push_back((float*)(c->ws + c->L.doms[k].kc));
+  int r = copy_field(c, bases.data(), kc.data(), false, false);
+  for (int a = 0; a < 3 && !r; ++a) {
+    std::vector<float*> bb;
+    for (size_t k = 0; k < c->doms.size(); ++k) bb.push_back((float*)(c->ws + c->L.doms[k].bq[a]));
+    r = copy_field(c, bb.data(), bq[a].data(), false, false);
+  }
+  if (r) return r;
+  for (size_t k = 0; k < c->doms.size(); ++k) {
+    DomainView& v = c->doms[k].v;
+    v.kc = bases[k];
+    for (int a = 0; a < 3; ++a) v.bq[a] = (const float*)(c->ws + c->L.doms[k].bq[a]);
+  }
+  return FDTD_OK;
+}
+
 int fdtd_set_model(fdtd_ctx* c, const float* c_host, const float* rho_host) {
   if (!c) return FDTD_EINVAL;
   const size_t n = (size_t)c->G.gn[0] * c->G.gn[1] * c->G.gn[2];
   double rho = 1.0;
   if (rho_host) {
     rho = rho_host[0];
-    for (size_t q = 1; q < n; ++q)
-      if (rho_host[q] != rho_host[0]) { set_err("heterogeneous density is not built (NEXT-3)"); return FDTD_EUNSUPPORTED; }
+    bool uniform = true;
+    for (size_t q = 1; q < n && uniform; ++q) uniform = rho_host[q] == rho_host[0];
+    if (!uniform) return set_model_density_array(c, c_host, rho_host);
     if (!(rho > 0.0)) { set_err("rho must be positive"); return FDTD_EINVAL; }
   }
+  for (auto& d : c->doms)
+    for (int a = 0; a < 3; ++a) d.v.bq[a] = nullptr;
   const float b0 = (float)(c->P.dt / (rho * c->P.dx));
   if (!c_host) {
     for (auto& d : c->doms) { d.v.kc = nullptr; d.v.kc0 = (float)(rho * 1.0 * 1.0 * c->P.dt / c->P.dx); d.v.b0 = b0; }

@@ -32,6 +32,7 @@ struct DomainView {
   float* f[4];             // p, vx, vy, vz
   const float* kc;         // K dt/dx per node (local layout) or nullptr -> kc0
   float kc0, b0;           // homogeneous K dt/dx and dt/(rho dx)
+  const float* bq[3];      // dt/(rho_bar dx) at the half nodes of vx, vy, vz (local layout) or nullptr -> b0 (R6)
   int ls[3][2], ln[3][2];  // CPML storage slabs in LOCAL indices: [axis][side] start, count (0 = none)
   float* psi[2][3][2];     // [family 0 = psi_v, 1 = psi_p][axis][side], slab-local
   const float* tab[2][3][3];  // [family][axis][a, b, 1/kappa], indexed by GLOBAL index along the axis
@@ -100,7 +101,7 @@ __global__ void __launch_bounds__(256) update_v_ref(DomainView D) {
       d = cpml_apply(d, s, D.tab[0][a][0][g[a]], D.tab[0][a][1][g[a]], D.tab[0][a][2][g[a]]);
       *ps = s;
     }
-    D.f[1 + a][q] = upd(D.f[1 + a][q], D.b0, d);
+    D.f[1 + a][q] = upd(D.f[1 + a][q], D.bq[a] ? D.bq[a][q] : D.b0, d);
   }
 }
 
@@ -294,6 +295,7 @@ __device__ __forceinline__ bool touches(const DomainView& D, int axis, int lo, i
 // On arrival of stage "p plane m": vx, vy of plane m are updated from the tile, p[m] enters the register queue and
 // vz of plane m-4 is updated from the queue (D+_z at k+1/2 reads p[k-3 .. k+4]).  The pinned last half node of each
 // axis (R3) is kept by a zero update coefficient (its psi stays 0 through a zero `a` in the device table).
+template <bool HB>
 __device__ __forceinline__ void v_item(const TMaps& tm, const DomainView& D, float* smem, const Ring& R, unsigned& it, int x0, int y0,
                                        int z0, int z1) {
   const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
@@ -324,6 +326,10 @@ __device__ __forceinline__ void v_item(const TMaps& tm, const DomainView& D, flo
   float* gvx = D.f[1] + rowoff + (long long)z0 * D.plane;
   float* gvy = D.f[2] + rowoff + (long long)z0 * D.plane;
   float* gvz = D.f[3] + rowoff + (long long)z0 * D.plane;
+  // heterogeneous density (HB): dt/(rho_bar dx) per half node, read straight from global memory (one reader per value)
+  const float* gbx = HB ? D.bq[0] + rowoff + (long long)z0 * D.plane : nullptr;
+  const float* gby = HB ? D.bq[1] + rowoff + (long long)z0 * D.plane : nullptr;
+  const float* gbz = HB ? D.bq[2] + rowoff + (long long)z0 * D.plane : nullptr;
   const int poff = (ty + 3) * HW + 4 * tx + 4;      // own float4 inside the p halo tile
   const int toff = ty * TX + 4 * tx;                // own float4 inside a plain tile
   // pinned last half nodes: zero coefficient
@@ -352,6 +358,11 @@ __device__ __forceinline__ void v_item(const TMaps& tm, const DomainView& D, flo
     if (xy && sx >= 0) { psx = ld4(ppx); prefetch_l2(ppx + PSI_AHEAD * stride_px); }
     if (xy && sy >= 0) { psy = ld4(ppy); prefetch_l2(ppy + PSI_AHEAD * stride_py); }
     if (sz >= 0 && active) { ppz = D.psi[0][2][sz] + psi_index(D, 2, sz, i, j, kz); psz = ld4(ppz); }
+    V4 bx4, by4, bz4;
+    if (HB) {
+      if (xy && active) { bx4 = ldg4(gbx); by4 = ldg4(gby); }
+      if (zz && active) bz4 = ldg4(gbz);
+    }
     // producer duty: refill the stage every warp released in the previous iteration
     if (tid == 0 && m > m_begin && (m - 1 + NS) < m_end) {
       const unsigned ps = (it - 1) % NS;
@@ -392,10 +403,21 @@ __device__ __forceinline__ void v_item(const TMaps& tm, const DomainView& D, flo
           ppy += stride_py;
         }
       }
-      vx4.v[0] = upd(vx4.v[0], B, dxv.v[0]); vx4.v[1] = upd(vx4.v[1], B, dxv.v[1]);
-      vx4.v[2] = upd(vx4.v[2], B, dxv.v[2]); vx4.v[3] = upd(vx4.v[3], Bx3, dxv.v[3]);
+      if (HB) {
+        const bool lastx = (i + 3 + D.ox) == D.gn[0] - 1, lasty = (j + D.oy) == D.gn[1] - 1;
 #pragma unroll
-      for (int e = 0; e < 4; ++e) vy4.v[e] = upd(vy4.v[e], By, dyv.v[e]);
+        for (int e = 0; e < 4; ++e) {
+          vx4.v[e] = upd(vx4.v[e], (e == 3 && lastx) ? 0.f : bx4.v[e], dxv.v[e]);
+          vy4.v[e] = upd(vy4.v[e], lasty ? 0.f : by4.v[e], dyv.v[e]);
+        }
+        gbx += D.plane;
+        gby += D.plane;
+      } else {
+        vx4.v[0] = upd(vx4.v[0], B, dxv.v[0]); vx4.v[1] = upd(vx4.v[1], B, dxv.v[1]);
+        vx4.v[2] = upd(vx4.v[2], B, dxv.v[2]); vx4.v[3] = upd(vx4.v[3], Bx3, dxv.v[3]);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) vy4.v[e] = upd(vy4.v[e], By, dyv.v[e]);
+      }
       if (active) { st4(gvx, vx4); st4(gvy, vy4); }
       gvx += D.plane;
       gvy += D.plane;
@@ -410,9 +432,10 @@ __device__ __forceinline__ void v_item(const TMaps& tm, const DomainView& D, flo
       }
       const float Bz = gk == D.gn[2] - 1 ? 0.f : B;
 #pragma unroll
-      for (int e = 0; e < 4; ++e) vz4.v[e] = upd(vz4.v[e], Bz, dzv.v[e]);
+      for (int e = 0; e < 4; ++e) vz4.v[e] = upd(vz4.v[e], HB ? (gk == D.gn[2] - 1 ? 0.f : bz4.v[e]) : Bz, dzv.v[e]);
       if (active) st4(gvz, vz4);
       gvz += D.plane;
+      if (HB) gbz += D.plane;
     }
   }
 }
@@ -438,6 +461,7 @@ __device__ __forceinline__ void ring_init(uint64_t* full, uint64_t* empty, unsig
   }
 }
 
+template <bool HB>
 __global__ void __launch_bounds__(NT, 2) update_v_tiled(const __grid_constant__ TMaps tm, const __grid_constant__ DomainView D,
                                                         const __grid_constant__ Sched S) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -449,7 +473,7 @@ __global__ void __launch_bounds__(NT, 2) update_v_tiled(const __grid_constant__ 
   const Ring R{full, empty};
   unsigned it = 0;
   int x0, y0, z0, z1;
-  while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) v_item(tm, D, smem, R, it, x0, y0, z0, z1);
+  while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) v_item<HB>(tm, D, smem, R, it, x0, y0, z0, z1);
 }
 
 // ---- pressure sub-update: p <- p - Kc [sum_a (1/kappa_a) D-_a v_a + psi_pa] for one item.

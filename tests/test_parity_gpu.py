@@ -209,6 +209,39 @@ def test_degenerate_grids_parity(B, kernel, shape, cpml):
     sim.destroy()
 
 
+@pytest.mark.parametrize("kernel", [1, 0])
+@pytest.mark.parametrize("shape,cpml", [((70, 45, 37), (5, 9, 0, 7, 6, 0)), ((124, 18, 21), (12, 12, 4, 4, 8, 8)), ((133, 18, 21), (0,) * 6)])
+def test_heterogeneous_density_parity(B, kernel, shape, cpml):
+    """SURVEY NEXT-3 (reading R6): rho(x) and c(x) both heterogeneous; dt/(rho_bar dx) at the half nodes."""
+    tot = tuple(shape[a] + cpml[2 * a] + cpml[2 * a + 1] for a in range(3))
+    rng = np.random.default_rng(3)
+    c = (1.0 + 0.3 * rng.random(tot[::-1])).astype(np.float32)
+    rho = (0.8 + 0.7 * rng.random(tot[::-1])).astype(np.float32)
+    kw = dict(dt=0.4 / 1.3, cpml_alpha_max=math.pi * inputs.F0, cpml_c_ref=1.3)
+    sim = B.Fdtd(shape, cpml, kernel=kernel, density=B.FDTD_DENSITY_ARRAY, **kw)
+    o = Oracle(shape, cpml, **kw)
+    sim.set_model(c, rho)
+    o.set_model(c, rho)
+    src = np.array([[tot[0] // 2, tot[1] // 3, tot[2] // 2]], np.int32)
+    wav = inputs.ricker(8, kw["dt"], t0=1.0)[None, :]
+    sim.set_sources(src, wav)
+    o.set_sources(src, wav)
+    for f in range(4):
+        sim.fill_hash(f, 42, 0.5)
+        o.fill_hash(f, 42, scale=0.5)
+    sim.step(8)
+    o.step(8)
+    for f in range(4):
+        assert rel(sim.get_field(f), o.get(f)) <= TOL, (f, rel(sim.get_field(f), o.get(f)))
+    for q in range(6):
+        assert rel(sim.get_psi(q), o.get(4 + q)) <= TOL, q
+    sim.set_model(c, np.full(tot[::-1], 2.0, np.float32))           # back to a uniform density: the scalar path again
+    sim.step(1)
+    sim.destroy()
+    with pytest.raises(B.FdtdError):                                # the single-pass step is not built for this
+        B.Fdtd((16,) * 3, dt=0.4, kernel=B.FDTD_KERNEL_FUSED, density=B.FDTD_DENSITY_ARRAY)
+
+
 def test_periodic_dispersion_on_gpu(B):
     """Pin P2 on the CUDA path (reference kernel, periodic): p^{n+1} + p^{n-1} = (2 - 4S) p^n."""
     N, mode = 16, (1, 2, 3)

@@ -64,6 +64,27 @@ def test_subdomains_bit_identical_fused(B, g, m):
         B.Fdtd(shape, cpml, dt=0.4, kernel=2, decomp=(1, 2, 2), ghost=4, substeps=1)   # odd m cannot be fused
 
 
+def test_subdomains_bit_identical_heterogeneous_medium(B):
+    """c(x) and rho(x) arrays in subdomain mode: every subdomain gets its window of the global coefficient arrays
+    (ghost cells included), so the fields match the monolithic run bit for bit."""
+    shape, cpml = (40, 56, 56), (4, 4, 8, 8, 8, 8)
+    tot = tuple(shape[a] + cpml[2 * a] + cpml[2 * a + 1] for a in range(3))
+    rng = np.random.default_rng(8)
+    c = (1.0 + 0.3 * rng.random(tot[::-1])).astype(np.float32)
+    rho = (0.8 + 0.7 * rng.random(tot[::-1])).astype(np.float32)
+    out = []
+    for kw in (dict(), dict(decomp=(1, 2, 2), ghost=8, substeps=2)):
+        sim = B.Fdtd(shape, cpml, dt=0.3, cpml_alpha_max=math.pi * inputs.F0, cpml_c_ref=1.3, density=B.FDTD_DENSITY_ARRAY, **kw)
+        sim.set_model(c, rho)
+        for f in range(4):
+            sim.fill_hash(f, 17, 0.5)
+        sim.step(12)
+        out.append([sim.get_field(f) for f in range(4)])
+        sim.destroy()
+    for a, b in zip(*out):
+        assert _same_bits(a, b)
+
+
 def test_insufficient_ghost_is_rejected(B):
     with pytest.raises(B.FdtdError):
         B.Fdtd((64,) * 3, (8,) * 6, dt=0.4, decomp=(1, 2, 2), ghost=8, substeps=3)
