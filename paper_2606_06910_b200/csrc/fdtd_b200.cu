@@ -975,9 +975,6 @@ int fdtd_cpml_table(fdtd_ctx* c, int32_t axis, int32_t half, float* a, float* b,
   return FDTD_OK;
 }
 
-#ifdef FDTD_TRACE
-int fdtd_debug_trace(long long* dst) { return cudaMemcpyFromSymbol(dst, fdtd::g_trace, sizeof(long long) * 12 * 64 * 6) == cudaSuccess ? 0 : -3; }
-#endif
 int fdtd_destroy(fdtd_ctx* c) {
   if (!c) return FDTD_EINVAL;
   cudaError_t e = cudaStreamSynchronize(c->stream);

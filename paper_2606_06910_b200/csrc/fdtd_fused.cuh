@@ -31,7 +31,7 @@ constexpr int FW_PROD = 4;                       // one warpgroup whose first la
                                                  // of the CTA (traced with clock64, see profiles/r01b_ncu_config3.md)
 constexpr int FNW = FW_MAIN + FW_HALO;           // 12 consumer warps
 constexpr int FNT = (FNW + FW_PROD) * 32;        // 512 threads = 4 warps per SM sub-partition
-constexpr int F_REGS_MAIN = 208, F_REGS_HALO = 72, F_REGS_PROD = 24;   // setmaxnreg split of 4 x 128 registers per sub-partition lane
+constexpr int F_REGS_MAIN = 200, F_REGS_HALO = 80, F_REGS_PROD = 32;   // setmaxnreg split of 4 x 128 registers per sub-partition lane
 constexpr int FNS = 4;                           // TMA ring stages
 constexpr int BW = TX + 16;                      // p box: columns x0-8 .. x0+TX+7
 constexpr int BH = TY + 14;                      // p box: rows    y0-7 .. y0+TY+6
@@ -57,12 +57,6 @@ struct OutSet {
   float* psi[2][3][2];
 };
 
-#ifdef FDTD_TRACE
-__device__ long long g_trace[12 * 64 * 6];
-#define TR(slot) do { if (blockIdx.x == 3 && (threadIdx.x & 31) == 0 && TR_E >= 300 && TR_E < 364) g_trace[((threadIdx.x >> 5) * 64 + (TR_E - 300)) * 6 + (slot)] = clock64(); } while (0)
-#else
-#define TR(slot) do {} while (0)
-#endif
 struct FusedBars {
   uint64_t* full;     // [FNS] TMA stage landed
   uint64_t* empty;    // [FNS] every warp has read the stage
@@ -148,8 +142,6 @@ __device__ __forceinline__ void fused_steady(const DomainView& D, const OutSet& 
   static_assert(R == 7, "canonical ring order: the rings are shifted, not renamed (an 8x unrolled body thrashes the 32 KB I-cache)");
   const unsigned slot = C.it % FNS;
   const float* st = smem + slot * F_STAGE_FLOATS;
-#define TR_E C.eit
-  TR(0);
   // psi of plane k arrived during the previous iteration; start the loads of plane k+1 now
   V4 psx, psy, ppx, ppy;
   if (XY) {
@@ -160,7 +152,6 @@ __device__ __forceinline__ void fused_steady(const DomainView& D, const OutSet& 
     }
   }
   if (!C.pre) mbar_wait(&Q.full[slot], (C.it / FNS) & 1);
-  TR(1);
   shift_push(C.pq, ld4(st + F_OFF_PT + K.toff));                // newest p_old plane: PQ(7)
   const float* row = st + K.boff;
   const V4 c = ld4(row);
@@ -193,7 +184,6 @@ __device__ __forceinline__ void fused_steady(const DomainView& D, const OutSet& 
   st4(E + K.exo, vx4);
   st4(E + K.eyo, vy4);
   warp_arrive(&Q.efull[eb]);
-  TR(2);
 
   // ---- vz_new at kz+1/2 from p_old[kz-3 .. kz+4], then D-_z of the new vz ring
   vz4 = fused_vz(D, O, K, C, PQ(0), PQ(1), PQ(2), PQ(3), PQ(4), PQ(5), PQ(6), PQ(7), vz4, k + 3);
@@ -206,10 +196,8 @@ __device__ __forceinline__ void fused_steady(const DomainView& D, const OutSet& 
   if (pz) ppz = K.active ? ldg4(D.psi[1][2][szp] + pozp) : zero4();
 
   // ---- pressure sub-update at plane k
-  TR(3);
   C.pre = mbar_test(&Q.full[(C.it + 1) % FNS], ((C.it + 1) / FNS) & 1);      // probe the next stage now, use the answer next iteration
   mbar_wait(&Q.efull[eb], (C.eit >> 1) & 1);
-  TR(4);
   const float* xr = E + K.exo;
   V4 dxp = diff_x<false>(ld4(xr - 4), vx4, ld4(xr + 4));
   const float* col = E + E_OFF_VY + K.ty * TX + 4 * K.tx;         // row ty of E.vy <-> y = j-4
@@ -236,9 +224,7 @@ __device__ __forceinline__ void fused_steady(const DomainView& D, const OutSet& 
   const V4 p4 = join2(__ffma2_rn(pk(-kc4.v[0], -kc4.v[1]), s0, lo2(PQ(0))), __ffma2_rn(pk(-kc4.v[2], -kc4.v[3]), s1, hi2(PQ(0))));
   if (K.active) st4(C.gp, p4);
   C.gvx += D.plane; C.gvy += D.plane; C.gp += D.plane;
-  TR(5);
   ++C.it; ++C.eit;
-#undef TR_E
 #undef PQ
 #undef WQ
 }
@@ -355,14 +341,11 @@ __device__ __forceinline__ void fused_halo(const TMaps& tm, const DomainView& D,
   for (int m = m_begin; m < m_end; ++m, ++it) {
     const unsigned slot = it % FNS;
     const bool out = (m - 7) >= z0;
-#define TR_E eit
-    if (out) TR(0);
     V4 psy, psx;
     if (out && sy >= 0) psy = ldg4(D.psi[0][1][sy] + poy);
     if (out && sx >= 0) psx = ldg4(D.psi[0][0][sx] + pox);
     const float* st = smem + slot * F_STAGE_FLOATS;
     mbar_wait(&Q.full[slot], (it / FNS) & 1);
-    if (out) TR(1);
     V4 dyv, vy4, dxv, vx4;
     if (out) {
       const float* rw = st + boff_y;
@@ -393,15 +376,11 @@ __device__ __forceinline__ void fused_halo(const TMaps& tm, const DomainView& D,
       float* E = ebuf + eb * E_FLOATS;
       // this buffer was last read for plane eit-2; every main warp is past that once the previous plane's efull phase
       // is complete (a main warp arrives there only after it has finished reading the plane before)
-      TR(3);
       if (eit > 0) mbar_wait(&Q.efull[eb ^ 1], ((eit - 1) >> 1) & 1);
-      TR(4);
       st4(E + E_OFF_VY + eyo, vy4);
       if (do_x) st4(E + exo, vx4);
       warp_arrive(&Q.efull[eb]);
-      TR(2);
       ++eit;
-#undef TR_E
     }
   }
 }
