@@ -33,9 +33,9 @@ def parse():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config3", choices=["config1", "config2", "config3", "config4"])
-    ap.add_argument("--kernel", default="two-pass", choices=["fused", "two-pass"],
-                    help="two-pass: update_v + update_p (48 B/pt, the default); fused: one single-pass launch per step "
-                         "(FDTD_KERNEL_FUSED, 32 B/pt, twice the field memory)")
+    ap.add_argument("--kernel", default="fused", choices=["fused", "two-pass"],
+                    help="fused: one single-pass launch per step (FDTD_KERNEL_FUSED, 32 B/pt, twice the field memory; the default); "
+                         "two-pass: update_v + update_p (48 B/pt)")
     ap.add_argument("--no-alt", action="store_true", help="do not also time the other kernel for the 'alt_kernel' entry")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")

@@ -377,12 +377,6 @@ __device__ __forceinline__ void v_item(const TMaps& tm, const DomainView& D, flo
       if (xy && active) { bx4 = ldg4(gbx); by4 = ldg4(gby); }
       if (zz && active) bz4 = ldg4(gbz);
     }
-    // producer duty: refill the stage every warp released in the previous iteration
-    if (tid == 0 && m > m_begin && (m - 1 + NS) < m_end) {
-      const unsigned ps = (it - 1) % NS;
-      mbar_wait(&R.empty[ps], ((it - 1) / NS) & 1);
-      issue(ps, m - 1 + NS);
-    }
     const float* st = smem + slot * V_STAGE_FLOATS;
     mbar_wait(&R.full[slot], (it / NS) & 1);
 
@@ -398,6 +392,14 @@ __device__ __forceinline__ void v_item(const TMaps& tm, const DomainView& D, flo
     }
     if (zz) vz4 = ld4(st + V_OFF_VZ + toff);
     release_stage(R, slot);
+    // producer duty, after this thread's own shared-memory loads of the iteration: a lane that has just issued tensor
+    // copies sees its next shared-memory loads stall for about a thousand cycles (traced on step_fused).  Refill the stage
+    // every warp released in the previous iteration.
+    if (tid == 0 && m > m_begin && (m - 1 + NS) < m_end) {
+      const unsigned ps = (it - 1) % NS;
+      mbar_wait(&R.empty[ps], ((it - 1) / NS) & 1);
+      issue(ps, m - 1 + NS);
+    }
     q0 = q1; q1 = q2; q2 = q3; q3 = q4; q4 = q5; q5 = q6; q6 = q7; q7 = c;     // q7 = p[m] ... q0 = p[m-7]
 
     if (xy) {
@@ -546,6 +548,7 @@ __device__ __forceinline__ void p_item(const TMaps& tm, const DomainView& D, flo
     if (out && sx >= 0) { psx = ld4(ppx); prefetch_l2(ppx + PSI_AHEAD * stride_px); }
     if (out && sy >= 0) { psy = ld4(ppy); prefetch_l2(ppy + PSI_AHEAD * stride_py); }
     if (sz >= 0 && active) { ppz = D.psi[1][2][sz] + psi_index(D, 2, sz, i, j, k); psz = ld4(ppz); }
+    // producer duty before the wait (measured: here the early refill is worth more than the stall it causes, unlike update_v)
     if (tid == 0 && m > m_begin && (m - 1 + NS) < m_end) {
       const unsigned ps = (it - 1) % NS;
       mbar_wait(&R.empty[ps], ((it - 1) / NS) & 1);
