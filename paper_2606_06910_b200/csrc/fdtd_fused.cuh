@@ -57,6 +57,28 @@ struct OutSet {
   float* psi[2][3][2];
 };
 
+// CPML tables of the item's columns x0-4 .. x0+TX+3 and rows y0-4 .. y0+TY+3 in shared memory ([family][a, b, 1/kappa]):
+// the per-plane table reads of the slab items were global loads issued right before their use (long-scoreboard stalls
+// in the source view); from here they are LDS next to the other shared-memory reads of the plane.
+constexpr int TCX = HW, TCY = TY + 8;
+struct TabCache {
+  float x[2][3][TCX];
+  float y[2][3][TCY];
+};
+// filled by all consumer threads of the CTA after next_item, then a named barrier among them (the producer group is not in it)
+__device__ __forceinline__ void fill_tab_cache(const DomainView& D, TabCache& T, int x0, int y0) {
+  for (int t = threadIdx.x; t < 6 * TCX; t += FNW * 32) {
+    const int col = t % TCX, ft = t / TCX;
+    const int g = min(max(x0 - 4 + col + D.ox, 0), D.gn[0] - 1);
+    T.x[ft / 3][ft % 3][col] = __ldg(D.tab[ft / 3][0][ft % 3] + g);
+  }
+  for (int t = threadIdx.x; t < 6 * TCY; t += FNW * 32) {
+    const int row = t % TCY, ft = t / TCY;
+    const int g = min(max(y0 - 4 + row + D.oy, 0), D.gn[1] - 1);
+    T.y[ft / 3][ft % 3][row] = __ldg(D.tab[ft / 3][1][ft % 3] + g);
+  }
+  asm volatile("bar.sync 1, %0;" ::"n"(FNW * 32) : "memory");
+}
 struct FusedBars {
   uint64_t* full;     // [FNS] TMA stage landed
   uint64_t* empty;    // [FNS] every warp has read the stage
@@ -104,6 +126,7 @@ struct MainConst {
   long long stride_px, stride_py, zrow;
   float Bxy, Bx3, By;
   bool active, has_kc;
+  const TabCache* T;
 };
 
 __device__ __forceinline__ void shift_push(V4 (&q)[8], const V4& v) {
@@ -167,11 +190,11 @@ __device__ __forceinline__ void fused_steady(const DomainView& D, const OutSet& 
   // ---- velocity sub-update at plane k
   if (XY) {
     if (K.sx >= 0) {
-      cpml4(dxv, psx, ldg4(D.tab[0][0][0] + K.gi), ldg4(D.tab[0][0][1] + K.gi), ldg4(D.tab[0][0][2] + K.gi));
+      cpml4(dxv, psx, ld4(K.T->x[0][0] + 4 + 4 * K.tx), ld4(K.T->x[0][1] + 4 + 4 * K.tx), ld4(K.T->x[0][2] + 4 + 4 * K.tx));
       st4(O.psi[0][0][K.sx] + C.pox, psx);
     }
     if (K.sy >= 0) {
-      cpml4s(dyv, psy, __ldg(D.tab[0][1][0] + K.gj), __ldg(D.tab[0][1][1] + K.gj), __ldg(D.tab[0][1][2] + K.gj));
+      cpml4s(dyv, psy, K.T->y[0][0][4 + K.ty], K.T->y[0][1][4 + K.ty], K.T->y[0][2][4 + K.ty]);
       st4(O.psi[0][1][K.sy] + C.poy, psy);
     }
   }
@@ -205,12 +228,12 @@ __device__ __forceinline__ void fused_steady(const DomainView& D, const OutSet& 
                   ld4(col));
   if (XY) {
     if (K.sx >= 0) {
-      cpml4(dxp, ppx, ldg4(D.tab[1][0][0] + K.gi), ldg4(D.tab[1][0][1] + K.gi), ldg4(D.tab[1][0][2] + K.gi));
+      cpml4(dxp, ppx, ld4(K.T->x[1][0] + 4 + 4 * K.tx), ld4(K.T->x[1][1] + 4 + 4 * K.tx), ld4(K.T->x[1][2] + 4 + 4 * K.tx));
       st4(O.psi[1][0][K.sx] + C.pox, ppx);
       C.pox += K.stride_px;
     }
     if (K.sy >= 0) {
-      cpml4s(dyp, ppy, __ldg(D.tab[1][1][0] + K.gj), __ldg(D.tab[1][1][1] + K.gj), __ldg(D.tab[1][1][2] + K.gj));
+      cpml4s(dyp, ppy, K.T->y[1][0][4 + K.ty], K.T->y[1][1][4 + K.ty], K.T->y[1][2][4 + K.ty]);
       st4(O.psi[1][1][K.sy] + C.poy, ppy);
       C.poy += K.stride_py;
     }
@@ -264,7 +287,7 @@ __device__ __forceinline__ void fused_main_item(const DomainView& D, const OutSe
 }
 
 __device__ __forceinline__ void fused_main(const DomainView& D, const OutSet& O, const float* smem, float* ebuf, const FusedBars& Q,
-                                           unsigned& it, unsigned& eit, int x0, int y0, int z0, int z1) {
+                                           const TabCache& T, unsigned& it, unsigned& eit, int x0, int y0, int z0, int z1) {
   const int tid = threadIdx.x;
   MainConst K;
   K.tx = tid & 15; K.ty = tid >> 4;
@@ -288,6 +311,7 @@ __device__ __forceinline__ void fused_main(const DomainView& D, const OutSet& O,
   K.stride_px = K.sx >= 0 ? (long long)D.ny * D.ln[0][K.sx] : 0;
   K.stride_py = K.sy >= 0 ? (long long)D.ln[1][K.sy] * D.pitch : 0;
   K.gi = K.i + D.ox; K.gj = K.j + D.oy;
+  K.T = &T;
   MainCtx C;
   C.it = it; C.eit = eit; C.pre = false;
   C.pox = K.sx >= 0 ? psi_index(D, 0, K.sx, K.i, K.j, z0) : 0;
@@ -304,7 +328,8 @@ __device__ __forceinline__ void fused_main(const DomainView& D, const OutSet& O,
 // Warp hw (0..3) computes vy_new on two of the rows y0-4..y0-1, y0+TY..y0+TY+2 (16 float4 units per row; the eighth
 // row slot is idle); warp 3 also computes vx_new on the strips x0-4..x0-1 and x0+TX..x0+TX+3 (rows y0..y0+TY-1).
 // Lane 0 of warp 0 is the TMA producer of the CTA.
-__device__ __forceinline__ void fused_halo(const TMaps& tm, const DomainView& D, float* smem, float* ebuf, const FusedBars& Q, unsigned it,
+__device__ __forceinline__ void fused_halo(const TMaps& tm, const DomainView& D, float* smem, float* ebuf, const FusedBars& Q,
+                                           const TabCache& T, unsigned it,
                                            unsigned eit, int hw, int x0, int y0, int z0, int z1) {
   const int lane = threadIdx.x & 31;
   const bool has_kc = D.kc != nullptr;
@@ -322,7 +347,6 @@ __device__ __forceinline__ void fused_halo(const TMaps& tm, const DomainView& D,
   const int sy = valid_y ? slab_side(D, 1, jy) : -1;
   long long poy = sy >= 0 ? psi_index(D, 1, sy, iy, jy, z0) : 0;
   const long long stride_py = sy >= 0 ? (long long)D.ln[1][sy] * D.pitch : 0;
-  const int gj = jy + D.oy;
   // vx unit of this lane (warp 3 only)
   const bool do_x = hw == FW_HALO - 1;
   const int row = lane >> 1, side = lane & 1;
@@ -335,15 +359,17 @@ __device__ __forceinline__ void fused_halo(const TMaps& tm, const DomainView& D,
   const int sx = valid_x ? slab_side(D, 0, xx) : -1;
   long long pox = sx >= 0 ? psi_index(D, 0, sx, xx, jx, z0) : 0;
   const long long stride_px = sx >= 0 ? (long long)D.ny * D.ln[0][sx] : 0;
-  const int gi = xx + D.ox;
+  const int xcol = side ? TX + 4 : 0;                        // the strip's first column in the table cache
   const int m_begin = z0 - 7, m_end = z1 + 7;
 
   for (int m = m_begin; m < m_end; ++m, ++it) {
     const unsigned slot = it % FNS;
     const bool out = (m - 7) >= z0;
     V4 psy, psx;
-    if (out && sy >= 0) psy = ldg4(D.psi[0][1][sy] + poy);
-    if (out && sx >= 0) psx = ldg4(D.psi[0][0][sx] + pox);
+    // psi of the ghost strips: read for this plane, pulled into L2 for a later one (the halo warps have about one plane of
+    // slack, which an unhidden DRAM latency per plane would use up in every slab item)
+    if (out && sy >= 0) { psy = ldg4(D.psi[0][1][sy] + poy); prefetch_l2(D.psi[0][1][sy] + poy + PSI_AHEAD * stride_py); }
+    if (out && sx >= 0) { psx = ldg4(D.psi[0][0][sx] + pox); prefetch_l2(D.psi[0][0][sx] + pox + PSI_AHEAD * stride_px); }
     const float* st = smem + slot * F_STAGE_FLOATS;
     mbar_wait(&Q.full[slot], (it / FNS) & 1);
     V4 dyv, vy4, dxv, vx4;
@@ -361,13 +387,13 @@ __device__ __forceinline__ void fused_halo(const TMaps& tm, const DomainView& D,
     warp_arrive(&Q.empty[slot]);
     if (out) {
       if (sy >= 0) {
-        cpml4s(dyv, psy, __ldg(D.tab[0][1][0] + gj), __ldg(D.tab[0][1][1] + gj), __ldg(D.tab[0][1][2] + gj));
+        cpml4s(dyv, psy, T.y[0][0][rr], T.y[0][1][rr], T.y[0][2][rr]);
         poy += stride_py;
       }
       vy4 = upd4(vy4, By, By, By, dyv);
       if (do_x) {
         if (sx >= 0) {
-          cpml4(dxv, psx, ldg4(D.tab[0][0][0] + gi), ldg4(D.tab[0][0][1] + gi), ldg4(D.tab[0][0][2] + gi));
+          cpml4(dxv, psx, ld4(T.x[0][0] + xcol), ld4(T.x[0][1] + xcol), ld4(T.x[0][2] + xcol));
           pox += stride_px;
         }
         vx4 = upd4(vx4, Bvx, Bvx, Bx3, dxv);
@@ -392,6 +418,7 @@ __global__ void __launch_bounds__(FNT, 1) step_fused(const __grid_constant__ TMa
   float* ebuf = smem + FNS * F_STAGE_FLOATS;
   __shared__ __align__(8) uint64_t bars[2 * FNS + 2];
   __shared__ int s_item;
+  __shared__ __align__(16) TabCache tabc;
   const FusedBars Q{bars, bars + FNS, bars + 2 * FNS};
   if (threadIdx.x == 0) {
 #pragma unroll
@@ -407,11 +434,15 @@ __global__ void __launch_bounds__(FNT, 1) step_fused(const __grid_constant__ TMa
   // warpgroups take the registers the halo warpgroup gives up (3 warps per SM sub-partition: 2 x 216 + 72 <= 512).
   if (warp < FW_MAIN) {
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(F_REGS_MAIN));
-    while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) fused_main(D, O, smem, ebuf, Q, it, eit, x0, y0, z0, z1);
+    while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) {
+      fill_tab_cache(D, tabc, x0, y0);
+      fused_main(D, O, smem, ebuf, Q, tabc, it, eit, x0, y0, z0, z1);
+    }
   } else if (warp < FNW) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(F_REGS_HALO));
     while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) {
-      fused_halo(tm, D, smem, ebuf, Q, it, eit, warp - FW_MAIN, x0, y0, z0, z1);
+      fill_tab_cache(D, tabc, x0, y0);
+      fused_halo(tm, D, smem, ebuf, Q, tabc, it, eit, warp - FW_MAIN, x0, y0, z0, z1);
       it += z1 - z0 + 14;
       eit += z1 - z0;
     }
