@@ -137,7 +137,8 @@ __device__ __forceinline__ void shift_push(V4 (&q)[8], const V4& v) {
 
 // vz_new[kz] from the p ring (logical order a[0..7] = p_old[kz-3 .. kz+4]), CPML in the z slabs, store if owned.
 __device__ __forceinline__ V4 fused_vz(const DomainView& D, const OutSet& O, const MainConst& K, MainCtx& C, const V4& a0, const V4& a1,
-                                       const V4& a2, const V4& a3, const V4& a4, const V4& a5, const V4& a6, const V4& a7, V4 vz4, int kz) {
+                                       const V4& a2, const V4& a3, const V4& a4, const V4& a5, const V4& a6, const V4& a7, V4 vz4, int kz,
+                                       const V4* early = nullptr) {
   V4 dzv = diff_8(a4, a3, a5, a2, a6, a1, a7, a0);
   const int gk = kz + D.oz;
   const bool inz = kz >= 0 && kz < D.nz;
@@ -145,7 +146,7 @@ __device__ __forceinline__ V4 fused_vz(const DomainView& D, const OutSet& O, con
     const int sz = kz < K.zl ? 0 : 1;
     const long long poz = (long long)(kz - D.ls[2][sz]) * D.plane + K.zrow;
     const float ta = __ldg(D.tab[0][2][0] + gk), tb = __ldg(D.tab[0][2][1] + gk), tk = __ldg(D.tab[0][2][2] + gk);
-    V4 psz = K.active ? ldg4(D.psi[0][2][sz] + poz) : zero4();
+    V4 psz = early ? *early : (K.active ? ldg4(D.psi[0][2][sz] + poz) : zero4());      // early: loaded at the top of the plane
     cpml4s(dzv, psz, ta, tb, tk);
     if (K.active && kz >= K.z0 && kz < K.z1) st4(O.psi[0][2][sz] + poz, psz);     // lead-in / tail planes belong to another item
   }
@@ -174,6 +175,14 @@ __device__ __forceinline__ void fused_steady(const DomainView& D, const OutSet& 
       if (K.sy >= 0) { C.nvy = ldg4(D.psi[0][1][K.sy] + C.poy + K.stride_py); C.npy = ldg4(D.psi[1][1][K.sy] + C.poy + K.stride_py); }
     }
   }
+  // psi of the z slabs (block-uniform per plane): issue the loads now, they are used after the velocity part
+  const int kzv = k + 3;
+  const bool zv = kzv < D.nz && (kzv < K.zl || kzv >= K.zh), pz = k < K.zl || k >= K.zh;
+  const int szv = kzv < K.zl ? 0 : 1, szp = k < K.zl ? 0 : 1;
+  const long long pozp = (long long)(k - D.ls[2][szp]) * D.plane + K.zrow;
+  V4 psz, ppz;
+  if (zv) psz = K.active ? ldg4(D.psi[0][2][szv] + (long long)(kzv - D.ls[2][szv]) * D.plane + K.zrow) : zero4();
+  if (pz) ppz = K.active ? ldg4(D.psi[1][2][szp] + pozp) : zero4();
   if (!C.pre) mbar_wait(&Q.full[slot], (C.it / FNS) & 1);
   shift_push(C.pq, ld4(st + F_OFF_PT + K.toff));                // newest p_old plane: PQ(7)
   const float* row = st + K.boff;
@@ -209,14 +218,9 @@ __device__ __forceinline__ void fused_steady(const DomainView& D, const OutSet& 
   warp_arrive(&Q.efull[eb]);
 
   // ---- vz_new at kz+1/2 from p_old[kz-3 .. kz+4], then D-_z of the new vz ring
-  vz4 = fused_vz(D, O, K, C, PQ(0), PQ(1), PQ(2), PQ(3), PQ(4), PQ(5), PQ(6), PQ(7), vz4, k + 3);
+  vz4 = fused_vz(D, O, K, C, PQ(0), PQ(1), PQ(2), PQ(3), PQ(4), PQ(5), PQ(6), PQ(7), vz4, kzv, zv ? &psz : nullptr);
   shift_push(C.wq, vz4);                                         // WQ(7) = vz_new[k+3]
   V4 dzp = diff_8(WQ(4), WQ(3), WQ(5), WQ(2), WQ(6), WQ(1), WQ(7), WQ(0));
-  V4 ppz;
-  const bool pz = k < K.zl || k >= K.zh;                         // block-uniform: plane k lies in a z slab
-  const int szp = k < K.zl ? 0 : 1;
-  const long long pozp = (long long)(k - D.ls[2][szp]) * D.plane + K.zrow;
-  if (pz) ppz = K.active ? ldg4(D.psi[1][2][szp] + pozp) : zero4();
 
   // ---- pressure sub-update at plane k
   C.pre = mbar_test(&Q.full[(C.it + 1) % FNS], ((C.it + 1) / FNS) & 1);      // probe the next stage now, use the answer next iteration
@@ -361,15 +365,20 @@ __device__ __forceinline__ void fused_halo(const TMaps& tm, const DomainView& D,
   const long long stride_px = sx >= 0 ? (long long)D.ny * D.ln[0][sx] : 0;
   const int xcol = side ? TX + 4 : 0;                        // the strip's first column in the table cache
   const int m_begin = z0 - 7, m_end = z1 + 7;
+  V4 npsy = zero4(), npsx = zero4();
+  if (sy >= 0) npsy = ldg4(D.psi[0][1][sy] + poy);
+  if (sx >= 0) npsx = ldg4(D.psi[0][0][sx] + pox);
 
   for (int m = m_begin; m < m_end; ++m, ++it) {
     const unsigned slot = it % FNS;
     const bool out = (m - 7) >= z0;
-    V4 psy, psx;
-    // psi of the ghost strips: read for this plane, pulled into L2 for a later one (the halo warps have about one plane of
-    // slack, which an unhidden DRAM latency per plane would use up in every slab item)
-    if (out && sy >= 0) { psy = ldg4(D.psi[0][1][sy] + poy); prefetch_l2(D.psi[0][1][sy] + poy + PSI_AHEAD * stride_py); }
-    if (out && sx >= 0) { psx = ldg4(D.psi[0][0][sx] + pox); prefetch_l2(D.psi[0][0][sx] + pox + PSI_AHEAD * stride_px); }
+    // psi of the ghost strips, loaded one plane ahead (the halo warps have about one plane of slack, which an unhidden
+    // DRAM latency per plane would use up in every slab item)
+    V4 psy = npsy, psx = npsx;
+    if (out && (m - 7) + 1 < z1) {
+      if (sy >= 0) npsy = ldg4(D.psi[0][1][sy] + poy + stride_py);
+      if (sx >= 0) npsx = ldg4(D.psi[0][0][sx] + pox + stride_px);
+    }
     const float* st = smem + slot * F_STAGE_FLOATS;
     mbar_wait(&Q.full[slot], (it / FNS) & 1);
     V4 dyv, vy4, dxv, vx4;

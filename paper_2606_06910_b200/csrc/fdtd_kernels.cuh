@@ -276,8 +276,9 @@ __device__ __forceinline__ V4 upd4(const V4& f, float c01, float c2, float c3, c
   return join2(__ffma2_rn(pk(-c01, -c01), lo2(d), lo2(f)), __ffma2_rn(pk(-c2, -c3), hi2(d), hi2(f)));
 }
 __device__ __forceinline__ void cpml4(V4& d, V4& ps, const V4& a, const V4& b, const V4& ik) {
-#pragma unroll
-  for (int e = 0; e < 4; ++e) d.v[e] = cpml_apply(d.v[e], ps.v[e], a.v[e], b.v[e], ik.v[e]);
+  const float2 p0 = __ffma2_rn(lo2(b), lo2(ps), __fmul2_rn(lo2(a), lo2(d))), p1 = __ffma2_rn(hi2(b), hi2(ps), __fmul2_rn(hi2(a), hi2(d)));
+  d = join2(__ffma2_rn(lo2(d), lo2(ik), p0), __ffma2_rn(hi2(d), hi2(ik), p1));
+  ps = join2(p0, p1);
 }
 __device__ __forceinline__ void cpml4s(V4& d, V4& ps, float a, float b, float ik) {
   const float2 a2 = pk(a, a), b2 = pk(b, b), k2 = pk(ik, ik);
