@@ -67,6 +67,8 @@ struct TabCache {
 };
 // filled by all consumer threads of the CTA after next_item, then a named barrier among them (the producer group is not in it)
 __device__ __forceinline__ void fill_tab_cache(const DomainView& D, TabCache& T, int x0, int y0) {
+  // block-uniform: nothing to do unless the tile or its ghost strips reach an x or y slab
+  if (!(touches(D, 0, x0 - 4, x0 + TX + 4) || touches(D, 1, y0 - 4, y0 + TY + 4))) return;
   for (int t = threadIdx.x; t < 6 * TCX; t += FNW * 32) {
     const int col = t % TCX, ft = t / TCX;
     const int g = min(max(x0 - 4 + col + D.ox, 0), D.gn[0] - 1);
@@ -137,8 +139,7 @@ __device__ __forceinline__ void shift_push(V4 (&q)[8], const V4& v) {
 
 // vz_new[kz] from the p ring (logical order a[0..7] = p_old[kz-3 .. kz+4]), CPML in the z slabs, store if owned.
 __device__ __forceinline__ V4 fused_vz(const DomainView& D, const OutSet& O, const MainConst& K, MainCtx& C, const V4& a0, const V4& a1,
-                                       const V4& a2, const V4& a3, const V4& a4, const V4& a5, const V4& a6, const V4& a7, V4 vz4, int kz,
-                                       const V4* early = nullptr) {
+                                       const V4& a2, const V4& a3, const V4& a4, const V4& a5, const V4& a6, const V4& a7, V4 vz4, int kz) {
   V4 dzv = diff_8(a4, a3, a5, a2, a6, a1, a7, a0);
   const int gk = kz + D.oz;
   const bool inz = kz >= 0 && kz < D.nz;
@@ -146,7 +147,7 @@ __device__ __forceinline__ V4 fused_vz(const DomainView& D, const OutSet& O, con
     const int sz = kz < K.zl ? 0 : 1;
     const long long poz = (long long)(kz - D.ls[2][sz]) * D.plane + K.zrow;
     const float ta = __ldg(D.tab[0][2][0] + gk), tb = __ldg(D.tab[0][2][1] + gk), tk = __ldg(D.tab[0][2][2] + gk);
-    V4 psz = early ? *early : (K.active ? ldg4(D.psi[0][2][sz] + poz) : zero4());      // early: loaded at the top of the plane
+    V4 psz = K.active ? ldg4(D.psi[0][2][sz] + poz) : zero4();
     cpml4s(dzv, psz, ta, tb, tk);
     if (K.active && kz >= K.z0 && kz < K.z1) st4(O.psi[0][2][sz] + poz, psz);     // lead-in / tail planes belong to another item
   }
@@ -175,14 +176,6 @@ __device__ __forceinline__ void fused_steady(const DomainView& D, const OutSet& 
       if (K.sy >= 0) { C.nvy = ldg4(D.psi[0][1][K.sy] + C.poy + K.stride_py); C.npy = ldg4(D.psi[1][1][K.sy] + C.poy + K.stride_py); }
     }
   }
-  // psi of the z slabs (block-uniform per plane): issue the loads now, they are used after the velocity part
-  const int kzv = k + 3;
-  const bool zv = kzv < D.nz && (kzv < K.zl || kzv >= K.zh), pz = k < K.zl || k >= K.zh;
-  const int szv = kzv < K.zl ? 0 : 1, szp = k < K.zl ? 0 : 1;
-  const long long pozp = (long long)(k - D.ls[2][szp]) * D.plane + K.zrow;
-  V4 psz, ppz;
-  if (zv) psz = K.active ? ldg4(D.psi[0][2][szv] + (long long)(kzv - D.ls[2][szv]) * D.plane + K.zrow) : zero4();
-  if (pz) ppz = K.active ? ldg4(D.psi[1][2][szp] + pozp) : zero4();
   if (!C.pre) mbar_wait(&Q.full[slot], (C.it / FNS) & 1);
   shift_push(C.pq, ld4(st + F_OFF_PT + K.toff));                // newest p_old plane: PQ(7)
   const float* row = st + K.boff;
@@ -218,9 +211,14 @@ __device__ __forceinline__ void fused_steady(const DomainView& D, const OutSet& 
   warp_arrive(&Q.efull[eb]);
 
   // ---- vz_new at kz+1/2 from p_old[kz-3 .. kz+4], then D-_z of the new vz ring
-  vz4 = fused_vz(D, O, K, C, PQ(0), PQ(1), PQ(2), PQ(3), PQ(4), PQ(5), PQ(6), PQ(7), vz4, kzv, zv ? &psz : nullptr);
+  vz4 = fused_vz(D, O, K, C, PQ(0), PQ(1), PQ(2), PQ(3), PQ(4), PQ(5), PQ(6), PQ(7), vz4, k + 3);
   shift_push(C.wq, vz4);                                         // WQ(7) = vz_new[k+3]
   V4 dzp = diff_8(WQ(4), WQ(3), WQ(5), WQ(2), WQ(6), WQ(1), WQ(7), WQ(0));
+  V4 ppz;
+  const bool pz = k < K.zl || k >= K.zh;                         // block-uniform: plane k lies in a z slab
+  const int szp = k < K.zl ? 0 : 1;
+  const long long pozp = (long long)(k - D.ls[2][szp]) * D.plane + K.zrow;
+  if (pz) ppz = K.active ? ldg4(D.psi[1][2][szp] + pozp) : zero4();
 
   // ---- pressure sub-update at plane k
   C.pre = mbar_test(&Q.full[(C.it + 1) % FNS], ((C.it + 1) / FNS) & 1);      // probe the next stage now, use the answer next iteration
