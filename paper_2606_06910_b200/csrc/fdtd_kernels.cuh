@@ -306,13 +306,25 @@ __device__ __forceinline__ bool touches(const DomainView& D, int axis, int lo, i
          (D.ln[axis][1] > 0 && lo < D.ls[axis][1] + D.ln[axis][1] && hi > D.ls[axis][1]);
 }
 
+// CPML tables [a, b, 1/kappa] of the item's 64 columns and 16 rows in shared memory: the per-plane global table loads sat
+// right before their use in the slab items (long-scoreboard stalls in the ncu source view of step_fused and of these).
+struct TabCache1 {
+  float x[3][TX];
+  float y[3][TY];
+};
+__device__ __forceinline__ void fill_tab_cache1(const DomainView& D, TabCache1& T, int fam, int x0, int y0) {
+  for (int t = threadIdx.x; t < 3 * TX; t += NT) T.x[t / TX][t % TX] = __ldg(D.tab[fam][0][t / TX] + min(x0 + t % TX + D.ox, D.gn[0] - 1));
+  for (int t = threadIdx.x; t < 3 * TY; t += NT) T.y[t / TY][t % TY] = __ldg(D.tab[fam][1][t / TY] + min(y0 + t % TY + D.oy, D.gn[1] - 1));
+  __syncthreads();
+}
+
 // ---- velocity sub-update: v_a <- v_a - B [(1/kappa_a) D+_a p + psi_va] for one item.
 // On arrival of stage "p plane m": vx, vy of plane m are updated from the tile, p[m] enters the register queue and
 // vz of plane m-4 is updated from the queue (D+_z at k+1/2 reads p[k-3 .. k+4]).  The pinned last half node of each
 // axis (R3) is kept by a zero update coefficient (its psi stays 0 through a zero `a` in the device table).
 template <bool HB>
-__device__ __forceinline__ void v_item(const TMaps& tm, const DomainView& D, float* smem, const Ring& R, unsigned& it, int x0, int y0,
-                                       int z0, int z1) {
+__device__ __forceinline__ void v_item(const TMaps& tm, const DomainView& D, float* smem, const Ring& R, TabCache1& T, unsigned& it, int x0,
+                                       int y0, int z0, int z1) {
   const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
   const int i = x0 + 4 * tx, j = y0 + ty;
   const int m_begin = z0 - 3, m_end = z1 + 4;
@@ -352,6 +364,7 @@ __device__ __forceinline__ void v_item(const TMaps& tm, const DomainView& D, flo
   const float By = (j + D.oy) == D.gn[1] - 1 ? 0.f : B;
   // CPML: block-uniform "does this item touch an x / y slab", per-thread "is my float4 / row inside one"
   const bool any_x = touches(D, 0, x0, x0 + TX), any_y = touches(D, 1, y0, y0 + TY);
+  if (any_x || any_y) fill_tab_cache1(D, T, 0, x0, y0);          // block-uniform
   const int sx = (any_x && active) ? slab_side(D, 0, i) : -1;
   const int sy = (any_y && active) ? slab_side(D, 1, j) : -1;
   float* ppx = sx >= 0 ? D.psi[0][0][sx] + psi_index(D, 0, sx, i, j, z0) : nullptr;
@@ -407,7 +420,7 @@ __device__ __forceinline__ void v_item(const TMaps& tm, const DomainView& D, flo
       if (any_x) {
         if (sx >= 0) {
           const int gi = i + D.ox;
-          cpml4(dxv, psx, ldg4(D.tab[0][0][0] + gi), ldg4(D.tab[0][0][1] + gi), ldg4(D.tab[0][0][2] + gi));
+          cpml4(dxv, psx, ld4(T.x[0] + 4 * tx), ld4(T.x[1] + 4 * tx), ld4(T.x[2] + 4 * tx));
           st4(ppx, psx);
           ppx += stride_px;
         }
@@ -415,7 +428,7 @@ __device__ __forceinline__ void v_item(const TMaps& tm, const DomainView& D, flo
       if (any_y) {
         if (sy >= 0) {
           const int gj = j + D.oy;
-          cpml4s(dyv, psy, __ldg(D.tab[0][1][0] + gj), __ldg(D.tab[0][1][1] + gj), __ldg(D.tab[0][1][2] + gj));
+          cpml4s(dyv, psy, T.y[0][ty], T.y[1][ty], T.y[2][ty]);
           st4(ppy, psy);
           ppy += stride_py;
         }
@@ -490,14 +503,15 @@ __global__ void __launch_bounds__(NT, 2) update_v_tiled(const __grid_constant__ 
   const Ring R{full, empty};
   unsigned it = 0;
   int x0, y0, z0, z1;
-  while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) v_item<HB>(tm, D, smem, R, it, x0, y0, z0, z1);
+  __shared__ __align__(16) TabCache1 tabc;
+  while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) v_item<HB>(tm, D, smem, R, tabc, it, x0, y0, z0, z1);
 }
 
 // ---- pressure sub-update: p <- p - Kc [sum_a (1/kappa_a) D-_a v_a + psi_pa] for one item.
 // Stage "vz plane m" also carries vx (x-halo tile), vy (y-halo tile), p and Kc of plane k = m-3; vz[m] enters the
 // register queue and p[k] is updated (D-_z at node k reads vz[k-4 .. k+3]).
-__device__ __forceinline__ void p_item(const TMaps& tm, const DomainView& D, float* smem, const Ring& R, unsigned& it, int x0, int y0,
-                                       int z0, int z1) {
+__device__ __forceinline__ void p_item(const TMaps& tm, const DomainView& D, float* smem, const Ring& R, TabCache1& T, unsigned& it, int x0,
+                                       int y0, int z0, int z1) {
   const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
   const int i = x0 + 4 * tx, j = y0 + ty;
   const int m_begin = z0 - 4, m_end = z1 + 3;
@@ -530,6 +544,7 @@ __device__ __forceinline__ void p_item(const TMaps& tm, const DomainView& D, flo
   const int toff = ty * TX + 4 * tx;                 // own float4 in a plain tile; row ty of the vy tile <-> y = y0-4+ty
   const float kc0 = D.kc0;
   const bool any_x = touches(D, 0, x0, x0 + TX), any_y = touches(D, 1, y0, y0 + TY);
+  if (any_x || any_y) fill_tab_cache1(D, T, 1, x0, y0);          // block-uniform
   const int sx = (any_x && active) ? slab_side(D, 0, i) : -1;
   const int sy = (any_y && active) ? slab_side(D, 1, j) : -1;
   float* ppx = sx >= 0 ? D.psi[1][0][sx] + psi_index(D, 0, sx, i, j, z0) : nullptr;
@@ -578,7 +593,7 @@ __device__ __forceinline__ void p_item(const TMaps& tm, const DomainView& D, flo
       if (any_x) {
         if (sx >= 0) {
           const int gi = i + D.ox;
-          cpml4(dxv, psx, ldg4(D.tab[1][0][0] + gi), ldg4(D.tab[1][0][1] + gi), ldg4(D.tab[1][0][2] + gi));
+          cpml4(dxv, psx, ld4(T.x[0] + 4 * tx), ld4(T.x[1] + 4 * tx), ld4(T.x[2] + 4 * tx));
           st4(ppx, psx);
           ppx += stride_px;
         }
@@ -586,7 +601,7 @@ __device__ __forceinline__ void p_item(const TMaps& tm, const DomainView& D, flo
       if (any_y) {
         if (sy >= 0) {
           const int gj = j + D.oy;
-          cpml4s(dyv, psy, __ldg(D.tab[1][1][0] + gj), __ldg(D.tab[1][1][1] + gj), __ldg(D.tab[1][1][2] + gj));
+          cpml4s(dyv, psy, T.y[0][ty], T.y[1][ty], T.y[2][ty]);
           st4(ppy, psy);
           ppy += stride_py;
         }
@@ -615,7 +630,8 @@ __global__ void __launch_bounds__(NT, 2) update_p_tiled(const __grid_constant__ 
   const Ring R{full, empty};
   unsigned it = 0;
   int x0, y0, z0, z1;
-  while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) p_item(tm, D, smem, R, it, x0, y0, z0, z1);
+  __shared__ __align__(16) TabCache1 tabc;
+  while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) p_item(tm, D, smem, R, tabc, it, x0, y0, z0, z1);
 }
 
 
