@@ -143,7 +143,7 @@ __device__ __forceinline__ V4 fused_vz(const DomainView& D, const OutSet& O, con
   V4 dzv = diff_8(a4, a3, a5, a2, a6, a1, a7, a0);
   const int gk = kz + D.oz;
   const bool inz = kz >= 0 && kz < D.nz;
-  if (inz && (kz < K.zl || kz >= K.zh)) {                      // block-uniform: this plane lies in a z slab
+  if (__builtin_expect(inz && (kz < K.zl || kz >= K.zh), 0)) {   // block-uniform: this plane lies in a z slab (few planes do)
     const int sz = kz < K.zl ? 0 : 1;
     const long long poz = (long long)(kz - D.ls[2][sz]) * D.plane + K.zrow;
     const float ta = __ldg(D.tab[0][2][0] + gk), tb = __ldg(D.tab[0][2][1] + gk), tk = __ldg(D.tab[0][2][2] + gk);
@@ -218,7 +218,7 @@ __device__ __forceinline__ void fused_steady(const DomainView& D, const OutSet& 
   const bool pz = k < K.zl || k >= K.zh;                         // block-uniform: plane k lies in a z slab
   const int szp = k < K.zl ? 0 : 1;
   const long long pozp = (long long)(k - D.ls[2][szp]) * D.plane + K.zrow;
-  if (pz) ppz = K.active ? ldg4(D.psi[1][2][szp] + pozp) : zero4();
+  if (__builtin_expect(pz, 0)) ppz = K.active ? ldg4(D.psi[1][2][szp] + pozp) : zero4();
 
   // ---- pressure sub-update at plane k
   C.pre = mbar_test(&Q.full[(C.it + 1) % FNS], ((C.it + 1) / FNS) & 1);      // probe the next stage now, use the answer next iteration
@@ -240,7 +240,7 @@ __device__ __forceinline__ void fused_steady(const DomainView& D, const OutSet& 
       C.poy += K.stride_py;
     }
   }
-  if (pz) {
+  if (__builtin_expect(pz, 0)) {
     const int gk = k + D.oz;
     cpml4s(dzp, ppz, __ldg(D.tab[1][2][0] + gk), __ldg(D.tab[1][2][1] + gk), __ldg(D.tab[1][2][2] + gk));
     if (K.active) st4(O.psi[1][2][szp] + pozp, ppz);
