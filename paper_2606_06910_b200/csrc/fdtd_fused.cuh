@@ -263,19 +263,21 @@ __device__ __forceinline__ void fused_main_item(const DomainView& D, const OutSe
   // lead-in 1: planes z0-7 .. z0-1 of p_old only fill the ring
   for (int m = z0 - 7; m < z0; ++m, ++C.it) {
     const unsigned slot = C.it % FNS;
-    mbar_wait(&Q.full[slot], (C.it / FNS) & 1);
+    if (!C.pre) mbar_wait(&Q.full[slot], (C.it / FNS) & 1);
     const V4 v = ld4(smem + slot * F_STAGE_FLOATS + F_OFF_PT + K.toff);
     warp_arrive(&Q.empty[slot]);
+    C.pre = mbar_test(&Q.full[(C.it + 1) % FNS], ((C.it + 1) / FNS) & 1);
     shift_push(C.pq, v);
   }
   // lead-in 2: planes z0 .. z0+6 also produce vz_new[z0-4 .. z0+2]
   for (int m = z0; m < z0 + 7; ++m, ++C.it) {
     const unsigned slot = C.it % FNS;
     const float* st = smem + slot * F_STAGE_FLOATS;
-    mbar_wait(&Q.full[slot], (C.it / FNS) & 1);
+    if (!C.pre) mbar_wait(&Q.full[slot], (C.it / FNS) & 1);
     const V4 v = ld4(st + F_OFF_PT + K.toff);
     V4 vz4 = ld4(st + F_OFF_VZ + K.toff);
     warp_arrive(&Q.empty[slot]);
+    C.pre = mbar_test(&Q.full[(C.it + 1) % FNS], ((C.it + 1) / FNS) & 1);
     shift_push(C.pq, v);
     vz4 = fused_vz(D, O, K, C, C.pq[0], C.pq[1], C.pq[2], C.pq[3], C.pq[4], C.pq[5], C.pq[6], C.pq[7], vz4, m - 4);
     shift_push(C.wq, vz4);
