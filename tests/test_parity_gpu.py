@@ -242,6 +242,27 @@ def test_heterogeneous_density_parity(B, kernel, shape, cpml):
         B.Fdtd((16,) * 3, dt=0.4, kernel=B.FDTD_KERNEL_FUSED, density=B.FDTD_DENSITY_ARRAY)
 
 
+def test_cpml_reflection_falls_with_thickness(B):
+    """P:170, Table 8 (trend only; the paper's procedure is unstated): against a reference run in a box so large
+    that nothing returns, a CPML-bounded run differs by orders of magnitude less than a wall-bounded one, and a thicker
+    layer reflects less.  Small version of paper_2606_06910_b200.reflection_study (kappa = 1 sets)."""
+    from paper_2606_06910_b200 import reflection_study as rs
+
+    interior, steps = 48, 200
+    pad = int(math.ceil(steps * inputs.COURANT * 1.3 / 2.0 / 4.0)) * 4 + 16
+    ref = rs.run(interior, 0, steps, 20, 20, pad, dict(), B.FDTD_KERNEL_AUTO)
+    shell = np.ones((interior,) * 3, bool)
+    shell[4:-4, 4:-4, 4:-4] = False
+    incident = max(float(np.abs(r[shell]).max()) for r in ref)
+    kw = dict(cpml_order=2, cpml_R0=1e-5, cpml_kappa_max=1.0, cpml_alpha_max=math.pi * inputs.F0)
+    ratio = {}
+    for L in (0, 8, 16):
+        t = rs.run(interior, L, steps, 20, 20, 0, kw if L else dict(), B.FDTD_KERNEL_FUSED if L == 16 else B.FDTD_KERNEL_AUTO)
+        ratio[L] = max(float(np.abs(a - b).max()) for a, b in zip(t, ref)) / incident
+    assert ratio[0] > 0.5                                   # walls send the pulse back
+    assert ratio[8] < 5e-3 and ratio[16] < ratio[8] / 3     # the layer absorbs it; a thicker one absorbs more
+
+
 def test_periodic_dispersion_on_gpu(B):
     """Pin P2 on the CUDA path (reference kernel, periodic): p^{n+1} + p^{n-1} = (2 - 4S) p^n."""
     N, mode = 16, (1, 2, 3)
