@@ -10,6 +10,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <string>
+#include <algorithm>
 #include <vector>
 
 using namespace fdtd;
@@ -144,6 +145,7 @@ struct Layout {
     uint64_t f[4], kc, psi[2][3][2], src_off, counters;
     uint64_t f2[4], psi2[2][3][2];   // fused mode: second state
     uint64_t bq[3];                  // FDTD_DENSITY_ARRAY: dt/(rho_bar dx) at the half nodes of vx, vy, vz
+    uint64_t items, items_cap;       // fused mode: item table of step_fused (int4 per item)
   };
   std::vector<Dom> doms;
   uint64_t tab[2][3][3];
@@ -189,6 +191,8 @@ Layout make_layout(const fdtd_params& P, const Geometry& G) {
           d.psi[fam][2][s] = take((uint64_t)d.pitch * d.n[1] * d.ln[2][s] * 4 + 16);
         }
       if (P.kernel == FDTD_KERNEL_FUSED) {
+        d.items_cap = (uint64_t)((d.n[0] + TX - 1) / TX) * ((d.n[1] + TY - 1) / TY) * (d.n[2] / 16 + 8);
+        d.items = take(d.items_cap * 16);
         for (int f = 0; f < 4; ++f) d.f2[f] = take(vol);
         for (int fam = 0; fam < 2; ++fam)
           for (int s = 0; s < 2; ++s) {
@@ -293,7 +297,10 @@ void plan_items(Domain& d, int grid) {
 }
 
 // step_fused items: the z lead-in of an item is 14 planes (7 of them load only a p tile), so chunks are long.
-void plan_items_fused(Domain& d, int grid) {
+// Items are handed out from a table, most expensive first (a tile x z-chunk that touches an x / y slab costs about 1.5x
+// an interior one per plane), with z-chunks that shrink from round to round, so that the CTAs finish together; within one
+// cost class the order stays x-fastest, so that concurrently running items are neighbours and share their halos in L2.
+void plan_items_fused(Domain& d, int grid, std::vector<int4>& table) {
   const DomainView& v = d.v;
   Sched& S = d.sched_f;
   S.ntx = (v.nx + TX - 1) / TX;
@@ -301,11 +308,36 @@ void plan_items_fused(Domain& d, int grid) {
   const long long tiles = (long long)S.ntx * S.nty;
   long long zc = (long long)v.nz * tiles / (12LL * std::max(grid, 1));
   zc = std::max(32LL, std::min(256LL, zc));
-  if (const char* e = getenv("FDTD_ZCHUNK_FUSED")) zc = std::max(1, atoi(e));
-  int n = (int)((v.nz + zc - 1) / zc);
-  S.zchunk = (v.nz + n - 1) / n;
-  S.nzc = (v.nz + S.zchunk - 1) / S.zchunk;
-  S.nitems = (int)(tiles * S.nzc);
+  bool uniform = false;
+  if (const char* e = getenv("FDTD_ZCHUNK_FUSED")) { zc = std::max(1, atoi(e)); uniform = true; }
+  // z-chunk boundaries: the first rounds take 1.5 zc planes, later ones shrink towards 32
+  std::vector<int> zb{0};
+  double sz = uniform ? (double)zc : 1.5 * (double)zc;
+  while (zb.back() < v.nz) {
+    int take = (int)std::max(uniform ? 1.0 : 32.0, sz);
+    if (v.nz - zb.back() - take < 24) take = v.nz - zb.back();          // no tiny last chunk: every chunk pays a 14-plane lead-in
+    zb.push_back(std::min(v.nz, zb.back() + take));
+    if (!uniform) sz *= 0.8;
+  }
+  auto touches_slab = [&](int axis, int lo, int hi) {
+    return (v.ln[axis][0] > 0 && lo < v.ls[axis][0] + v.ln[axis][0] && hi > v.ls[axis][0]) ||
+           (v.ln[axis][1] > 0 && lo < v.ls[axis][1] + v.ln[axis][1] && hi > v.ls[axis][1]);
+  };
+  struct Item { double cost; int4 t; };
+  std::vector<Item> items;
+  for (size_t c = 0; c + 1 < zb.size(); ++c)
+    for (int ty = 0; ty < S.nty; ++ty)
+      for (int tx = 0; tx < S.ntx; ++tx) {
+        const int x0 = tx * TX, y0 = ty * TY;
+        const bool slab = touches_slab(0, x0, x0 + TX) || touches_slab(1, y0, y0 + TY);
+        items.push_back({(zb[c + 1] - zb[c] + 4) * (slab ? 1.5 : 1.0), make_int4(x0, y0, zb[c], zb[c + 1])});
+      }
+  if (!uniform) std::stable_sort(items.begin(), items.end(), [](const Item& a, const Item& b) { return a.cost > b.cost; });
+  table.clear();
+  for (auto& it : items) table.push_back(it.t);
+  S.zchunk = (int)zc;
+  S.nzc = (int)zb.size() - 1;
+  S.nitems = (int)table.size();
 }
 
 // One fused time step of one domain: state v.f / v.psi -> d.alt, then the two are swapped.
@@ -668,7 +700,16 @@ fdtd_ctx* fdtd_create(const fdtd_params* P) {
       if ((e = cudaFuncSetAttribute(step_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, F_SMEM_BYTES)) != cudaSuccess)
         return fail(c, e, "cudaFuncSetAttribute(step_fused)");
       if (plan_launch(c, (const void*)step_fused, F_SMEM_BYTES, &c->grid_f, FNT)) { delete c; return nullptr; }
-      for (auto& d : c->doms) plan_items_fused(d, c->grid_f);
+      for (size_t k = 0; k < c->doms.size(); ++k) {
+        Domain& d = c->doms[k];
+        std::vector<int4> table;
+        plan_items_fused(d, c->grid_f, table);
+        if (table.size() > L.doms[k].items_cap) { set_err("item table larger than its workspace slot"); delete c; return nullptr; }
+        if ((e = cudaMemcpyAsync(c->ws + L.doms[k].items, table.data(), table.size() * sizeof(int4), cudaMemcpyHostToDevice, c->stream)) != cudaSuccess ||
+            (e = cudaStreamSynchronize(c->stream)) != cudaSuccess)
+          return fail(c, e, "cudaMemcpyAsync(item table)");
+        d.sched_f.table = (const int4*)(c->ws + L.doms[k].items);
+      }
     }
   }
   return c;

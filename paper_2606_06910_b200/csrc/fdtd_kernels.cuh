@@ -228,6 +228,7 @@ struct Sched {
   int nitems;
   unsigned int* counter;       // this launch's work counter
   unsigned int* other;         // the counter of the next launch on this domain: reset here
+  const int4* table;           // optional: item -> (x0, y0, z0, z1) in the order they are handed out (nullptr: tile-major decode)
 };
 
 // Four consecutive x values held in registers; moved as one 128-bit access.
@@ -478,6 +479,11 @@ __device__ __forceinline__ bool next_item(const Sched& S, int* s_item, int& x0, 
   __syncthreads();
   const int item = *s_item;
   if (item >= S.nitems) return false;
+  if (S.table) {
+    const int4 t = __ldg(S.table + item);
+    x0 = t.x; y0 = t.y; z0 = t.z; z1 = t.w;
+    return true;
+  }
   const int txi = item % S.ntx, r = item / S.ntx;
   const int tyi = r % S.nty, zc = r / S.nty;
   x0 = txi * TX; y0 = tyi * TY; z0 = zc * S.zchunk; z1 = min(z0 + S.zchunk, nz);
