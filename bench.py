@@ -1,13 +1,17 @@
 #!/usr/bin/env python
 """bench.py — throughput of the FDTD + CPML time step on B200, and the oracle beside it.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config3|config2|config4|config1]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config4|config3|config2|config1]
   python bench.py --impl reference ...        # the CPU oracle, as it stands, on a bounded sample of the same workload
 
 A "step" is one time step of the whole hot path (velocity sub-update, pressure sub-update, source; SURVEY 8a rows
 a1-a5) over the whole grid.  metric = Mpoints/s = Nx Ny Nz steps / (1e6 T) counting interior + CPML cells
-(PAPER.md P:228).  One process per GPU; N > 1 runs N independent replicas (the path does not shard: DESIGN.md
-"Multi-GPU"), value = points of all ranks / max-over-ranks time.  Prints ONE JSON line on rank 0.
+(PAPER.md P:228).  The default workload is BASELINE config 4 (1600^3 total), the largest single-GPU configuration;
+configs 3 and 2 are timed in the same run and carried under "other_workloads".  The timed region of K steps is repeated
+5 times (CUDA events, barrier + synchronize on both sides); value / ms_per_step are the median repeat (the paper
+reports medians), min and max are printed beside it.  One process per GPU; N > 1 runs N independent
+replicas (the path does not shard: DESIGN.md "Multi-GPU"), value = points of all ranks / max-over-ranks time.
+Prints ONE JSON line on rank 0.
 """
 import argparse
 import json
@@ -29,10 +33,12 @@ UNIT = "Mpts/s"
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
-    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=40)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--repeats", type=int, default=5, help="timed regions of K steps; the median is reported")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="config3", choices=["config1", "config2", "config3", "config4"])
+    ap.add_argument("--workload", default="config4", choices=["config1", "config2", "config3", "config4"])
+    ap.add_argument("--no-others", action="store_true", help="do not also time the other BASELINE workloads and the CPML-off runs")
     ap.add_argument("--kernel", default="fused", choices=["fused", "two-pass"],
                     help="fused: one single-pass launch per step (FDTD_KERNEL_FUSED, 32 B/pt, twice the field memory; the default); "
                          "two-pass: update_v + update_p (48 B/pt)")
@@ -77,7 +83,8 @@ def algorithmic_bytes(w):
 
 
 def ncu_traffic(wname):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture (profiles/*.csv)."""
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch as recorded by a committed `ncu --set full` capture
+    (profiles/dram_traffic.csv: kernel, workload, bytes, source file).  Not measured by this run: -> {kernel: (bytes, source)}."""
     path = os.path.join(ROOT, "profiles", "dram_traffic.csv")
     if not os.path.exists(path):
         return {}
@@ -86,9 +93,9 @@ def ncu_traffic(wname):
         for line in f:
             if line.startswith("#") or not line.strip():
                 continue
-            k, wl, b = line.strip().split(",")[:3]
+            k, wl, b, src = (line.strip().split(",") + [""])[:4]
             if wl == wname:
-                out[k] = float(b)
+                out[k] = (float(b), src)
     return out
 
 
@@ -117,7 +124,7 @@ class ClockSampler:
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
-                                       "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+                                       "-lms", "20"], stdout=self.f, stderr=subprocess.DEVNULL)
         except OSError:
             self.p = None
 
@@ -240,10 +247,9 @@ def main():
 
     from paper_2606_06910_b200 import binding
 
-    K, W = args.steps, max(args.warmup, 3)
-    w = workload(args.workload, 2 * K + W)
-    if args.cpml_off:
-        w.n_interior, w.cpml = w.total, (0,) * 6
+    K, W, R = args.steps, max(args.warmup, 3), max(args.repeats, 1)
+    total_steps = W + (R + 1) * K + 8
+    peak, peak_src = peaks()
 
     def barrier():
         if world > 1:
@@ -252,102 +258,172 @@ def main():
 
     fused = args.kernel == "fused"
     kern = binding.FDTD_KERNEL_FUSED if fused else binding.FDTD_KERNEL_AUTO
+    kname = {binding.FDTD_KERNEL_FUSED: "fused", binding.FDTD_KERNEL_AUTO: "two-pass"}
 
-    def timed_run(kernel, sample_clocks):
-        """W warm-up steps, then K steps between two CUDA events (barrier + synchronize on both sides), then the same
-        K steps again with an event after every launch group for the per-kernel split."""
+    def timed_run(w, kernel, sample_clocks=False):
+        """W warm-up steps, then R regions of K steps, each between two CUDA events with barrier + synchronize on both sides;
+        then K more steps with an event after every launch group (the per-kernel split; it carries event overhead)."""
         sim = binding.from_workload(w, device=local, kernel=kernel)
-        for f in range(1, 4):                   # non-trivial state everywhere (values do not change the traffic)
+        for f in range(4):                      # non-trivial state everywhere: the values decide the power drawn, not the traffic
             sim.fill_hash(f, 99, 1e-3)
+        sampler = ClockSampler(local) if (rank == 0 and sample_clocks) else None      # started before the warm-up
         sim.step(W)
-        barrier()
-        sampler = ClockSampler(local) if (rank == 0 and sample_clocks) else None
-        l0 = sim.launch_count()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        sim.step(K)
-        e1.record()
-        barrier()
-        t = e0.elapsed_time(e1)
-        n_launch = sim.launch_count() - l0
-        split = sim.step_profiled(K)
+        times, n_launch = [], 0
+        for _ in range(R):
+            barrier()
+            l0 = sim.launch_count()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            sim.step(K)
+            e1.record()
+            barrier()
+            times.append(max_over_ranks(e0.elapsed_time(e1), world, "cuda"))
+            n_launch = sim.launch_count() - l0
         clk = sampler.stop() if sampler else None
-        t = max_over_ranks(t, world, "cuda")
+        split = sim.step_profiled(K)
         sim.destroy()
         del sim
         torch.cuda.empty_cache()
-        return t, n_launch, split, clk
+        ms = float(np.median(times))
+        return {"ms": ms, "times": times, "launches": n_launch, "split": split, "clocks": clk}
 
-    ms, launches, prof, clocks = timed_run(kern, True)
+    def summarise(w, run, kernel):
+        """value, ms/step and the roofline of the step structure that ran, from the median back-to-back region."""
+        bv, bp, bf = algorithmic_bytes(w)
+        is_f = kernel == binding.FDTD_KERNEL_FUSED
+        step_bytes = bf if is_f else bv + bp
+        ms_step = run["ms"] / K
+        gbps = step_bytes / (ms_step * 1e-3) / 1e9
+        return {"kernel": kname[kernel], "value": throughput_mpts(w.points, K, world, run["ms"] * 1e-3), "unit": UNIT, "ms_per_step": ms_step,
+                "ms_per_step_min": min(run["times"]) / K, "ms_per_step_max": max(run["times"]) / K,
+                "step_bytes": step_bytes, "step_GBps": gbps, "step_frac_of_peak": gbps / peak, "step_frac_of_8000": gbps / 8000.0}
+
+    def cpml_off(w):
+        import copy
+        o = copy.copy(w)
+        o.n_interior, o.cpml = w.total, (0,) * 6
+        return o
+
+    w = workload(args.workload, total_steps)
+    if args.cpml_off:
+        w = cpml_off(w)
+    main_run = timed_run(w, kern, sample_clocks=True)
+    ms, launches, prof, clocks = main_run["ms"], main_run["launches"], main_run["split"], main_run["clocks"]
+
     alt = None
     if not args.no_alt and w.total[0] % 4 == 0:
         other = binding.FDTD_KERNEL_AUTO if fused else binding.FDTD_KERNEL_FUSED
-        a_ms, _, a_prof, _ = timed_run(other, False)
-        alt = {"kernel": "two-pass" if fused else "fused", "value": throughput_mpts(w.points, K, world, a_ms * 1e-3), "unit": UNIT,
-               "ms_per_step": a_ms / K, "kernels_ms_per_step": {("step_fused" if (k == "update_v" and not fused) else k): v / K for k, v in a_prof.items() if v > 0}}
+        a_run = timed_run(w, other)
+        alt = summarise(w, a_run, other)
+        alt["kernels_ms_per_step_profiled"] = {("step_fused" if (k == "update_v" and not fused) else k): v / K for k, v in a_run["split"].items() if v > 0}
 
-    # ---- end to end through the C ABI with host buffers: model up, K steps, pressure field down
+    # CPML overhead of the headline workload (R23: same total grid, plain walls), same kernel
+    overhead = None
+    if not args.no_others and not args.cpml_off and world == 1:
+        o_run = timed_run(cpml_off(w), kern)
+        overhead = {"cpml_off_ms_per_step": o_run["ms"] / K, "cpml_off_value": throughput_mpts(w.points, K, world, o_run["ms"] * 1e-3),
+                    "overhead": ms / o_run["ms"] - 1.0, "psi_byte_floor": 16.0 * slab_points(w) / ((32 if fused else 48) * w.points + (4 * w.points if w.c is not None else 0))}
+
+    # ---- end to end through the C ABI with host buffers: the same state as the timed leg (counter-based fill, set up
+    # before the clock starts), then inside the timed region: model up from pinned host memory, sources up, K steps,
+    # pressure field down into pinned host memory.
     e2e = None
     if not args.no_e2e:
         n = w.points
-        c_host = None
-        if w.c is not None:
-            c_host = torch.from_numpy(w.c).pin_memory()
+        c_host = torch.tensor(w.c).pin_memory() if w.c is not None else None
         out_host = torch.empty(n, dtype=torch.float32).pin_memory()
-        sim = binding.Fdtd(w.n_interior, w.cpml, device=local, kernel=kern, **w.cpml_kwargs())
+        sim = binding.Fdtd(w.n_interior, w.cpml, device=local, kernel=kern,
+                           medium=binding.FDTD_MEDIUM_ARRAY if w.c is not None else binding.FDTD_MEDIUM_UNIFORM, **w.cpml_kwargs())
+        for f in range(4):
+            sim.fill_hash(f, 99, 1e-3)
+        sim.step(W)                              # warm: the same clocks and power state as the timed leg
         barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         t0 = time.perf_counter()
         if c_host is not None:
             sim.set_model_from(c_host.data_ptr())
         sim.set_sources(w.sources, w.wavelets)
+        e0.record()
         sim.step(K)
+        e1.record()
         sim.get_field_into(binding.FDTD_P, out_host.data_ptr())
         torch.cuda.synchronize()
         dt_e = time.perf_counter() - t0
+        step_s = e0.elapsed_time(e1) * 1e-3
         dt_e = max_over_ranks(dt_e, world, "cuda")
         h2d = (n * 4 if c_host is not None else 0) + w.sources.nbytes + w.wavelets.nbytes
         e2e = {"value": throughput_mpts(n, K, world, dt_e), "unit": UNIT, "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": n * 4 / K,
-               "seconds": dt_e, "what": "fdtd_set_model + fdtd_set_sources + fdtd_step(K) + fdtd_get_field(p), pinned host buffers"}
+               "seconds": dt_e, "step_seconds": step_s, "copy_seconds": dt_e - step_s,
+               "d2h_GBps": n * 4 / max(dt_e - step_s, 1e-9) / 1e9 if c_host is None else None,
+               "what": "fdtd_set_model + fdtd_set_sources + fdtd_step(K) + fdtd_get_field(p) on the warmed, hash-filled state of the timed leg; "
+                       "pinned host buffers; copy_seconds = seconds - step_seconds (CUDA events around the K steps)"}
         sim.destroy()
-        del sim
+        del sim, out_host, c_host
+        torch.cuda.empty_cache()
+
+    # ---- the other BASELINE workloads in the same run (parity-test configurations, reported for context): both step
+    # structures, and the CPML-off run of R23 for the overhead BASELINE config 2 asks for
+    others = None
+    if not args.no_others and not args.cpml_off and world == 1:
+        others = {}
+        for name in ("config3", "config2"):
+            if name == args.workload:
+                continue
+            ow = workload(name, total_steps)
+            r_on = timed_run(ow, kern)
+            r_off = timed_run(cpml_off(ow), kern)
+            r_alt = timed_run(ow, binding.FDTD_KERNEL_AUTO if fused else binding.FDTD_KERNEL_FUSED)
+            ent = summarise(ow, r_on, kern)
+            ent["total_grid"] = list(ow.total)
+            ent["cpml_off_ms_per_step"] = r_off["ms"] / K
+            ent["cpml_overhead"] = r_on["ms"] / r_off["ms"] - 1.0
+            ent["psi_byte_floor"] = 16.0 * slab_points(ow) / ((32 if fused else 48) * ow.points + (4 * ow.points if ow.c is not None else 0))
+            ent["alt_kernel"] = summarise(ow, r_alt, binding.FDTD_KERNEL_AUTO if fused else binding.FDTD_KERNEL_FUSED)
+            others[name] = ent
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return 0
 
-    value = throughput_mpts(w.points, K, world, ms * 1e-3)
+    head = summarise(w, main_run, kern)
     bv, bp, bf = algorithmic_bytes(w)
-    peak, peak_src = peaks()
+    tot_prof = sum(prof.values())
     if fused:
-        dom, dur, byt, step_bytes = "step_fused", prof["update_v"] / K * 1e-3, bf, bf
+        dom, byt, share = "step_fused", bf, prof["update_v"] / tot_prof
         prof = {"step_fused": prof["update_v"], "inject": prof["inject"], "exchange": prof["exchange"]}
     else:
         dom = "update_v_tiled" if prof["update_v"] >= prof["update_p"] else "update_p_tiled"
-        dur = (prof["update_v"] if dom == "update_v_tiled" else prof["update_p"]) / K * 1e-3
-        byt, step_bytes = (bv if dom == "update_v_tiled" else bp), bv + bp
-    traffic = ncu_traffic(w.name)
-    step_gbps = step_bytes / (ms * 1e-3 / K) / 1e9
+        share = (prof["update_v"] if dom == "update_v_tiled" else prof["update_p"]) / tot_prof
+        byt = bv if dom == "update_v_tiled" else bp
+    dur = head["ms_per_step"] * 1e-3 * share             # the kernel's share of the back-to-back step time
+    traffic = ncu_traffic(w.name).get(dom)
     roof = {"bound": "hbm", "kernel": dom, "achieved": byt / dur / 1e9, "peak": peak, "unit": "GB/s",
-            "frac": byt / dur / 1e9 / peak, "peak_source": peak_src, "traffic": traffic.get(dom),
+            "frac": byt / dur / 1e9 / peak, "frac_of_8000": byt / dur / 1e9 / 8000.0, "peak_source": peak_src,
+            "traffic": traffic[0] if traffic else None,
+            "traffic_source": ("committed ncu --set full capture, not this run: profiles/" + traffic[1]) if traffic else None,
             "algorithmic_bytes_per_launch": byt, "avg_launch_ms": dur * 1e3,
-            "step": {"bytes": step_bytes, "model": "single pass, 32 B/pt + Kc + psi" if fused else "two passes, 48 B/pt + Kc + psi",
-                     "GBps": step_gbps, "frac": step_gbps / peak, "frac_of_8000": step_gbps / 8000.0,
-                     "two_pass_equivalent_GBps": (bv + bp) / (ms * 1e-3 / K) / 1e9},
-            "kernels_ms_per_step": {k: v / K for k, v in prof.items()}}
+            "avg_launch_ms_source": "median back-to-back ms_per_step x the kernel's share of the event-profiled split",
+            "kernel_share_of_step": share,
+            "step": {"bytes": head["step_bytes"], "model": "single pass, 32 B/pt + Kc + psi" if fused else "two passes, 48 B/pt + Kc + psi",
+                     "GBps": head["step_GBps"], "frac": head["step_frac_of_peak"], "frac_of_8000": head["step_frac_of_8000"],
+                     "two_pass_equivalent_GBps": (bv + bp) / (head["ms_per_step"] * 1e-3) / 1e9},
+            "kernels_ms_per_step_profiled": {k: v / K for k, v in prof.items()},
+            "profiled_note": "one CUDA event after every launch: about 2 % slower than back to back"}
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
+        "metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": head["ms_per_step"],
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": w.name + ("-cpml-off" if args.cpml_off else ""), "total_grid": list(w.total), "cpml": list(w.cpml),
                    "medium": "heterogeneous c (Kc array)" if w.c is not None else "homogeneous", "sources": int(w.sources.shape[0]),
-                   "kernel": args.kernel, "parallelism": "replicas x%d" % world, "l2": "inputs larger than L2 (fields %.1f GB)" % (w.points * 16 / 1e9)},
-        "roofline": roof, "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e, "alt_kernel": alt,
+                   "kernel": args.kernel, "parallelism": "replicas x%d" % world, "l2": "inputs larger than L2 (fields %.1f GB)" % (w.points * 16 / 1e9),
+                   "state": "counter-based random fields (scale 1e-3) + the config's sources"},
+        "repeats": {"n": R, "statistic": "median", "ms_per_step": [t / K for t in main_run["times"]],
+                    "min": head["ms_per_step_min"], "max": head["ms_per_step_max"]},
+        "roofline": roof, "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e, "alt_kernel": alt, "cpml": overhead,
+        "other_workloads": others,
     }
-    if alt is not None:
-        ab = (bv + bp) if fused else bf                # algorithmic bytes of the other kernel structure
-        alt["step_frac_of_peak"] = ab / (alt["ms_per_step"] * 1e-3) / 1e9 / peak
     if not args.no_cpu_baseline and world == 1:
-        line["cpu_baseline"] = oracle_sample(w, 24)
+        line["cpu_baseline"] = oracle_sample(w, 300)        # about 12 s on 16 cores
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

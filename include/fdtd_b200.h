@@ -45,6 +45,12 @@ enum {
                             /* per point), so fdtd_set_model accepts a heterogeneous rho (R6)     */
 };
 enum {
+  FDTD_MEDIUM_ARRAY = 0,  /* the workspace holds a per-node K dt/dx array (+4 B per point), so fdtd_set_model accepts a   */
+                          /* wave-speed array c(x) (BASELINE config 3)                                                   */
+  FDTD_MEDIUM_UNIFORM = 1 /* c is one number: no per-node array is reserved (saves one field: 16.4 GB at 1600^3);        */
+                          /* fdtd_set_model with a c array then returns FDTD_EUNSUPPORTED                                */
+};
+enum {
   FDTD_KERNEL_AUTO = 0, /* TMA-staged, z-streaming tile kernels (the product path)                        */
   FDTD_KERNEL_REF = 1,  /* one thread per point, global loads only; also the only path for FDTD_PERIODIC   */
   FDTD_KERNEL_FUSED = 2 /* one launch per time step: both sub-updates in a single pass over the fields (32 B  */
@@ -70,7 +76,8 @@ typedef struct {
   int32_t ghost;          /* ghost depth g in cells on every internal interface                 */
   int32_t substeps_per_exchange; /* m sub-updates (v or p) between halo exchanges; needs g >= 4 m (R20)      */
   int32_t kernel;         /* FDTD_KERNEL_AUTO / FDTD_KERNEL_REF / FDTD_KERNEL_FUSED                          */
-  int32_t density;        /* FDTD_DENSITY_UNIFORM / FDTD_DENSITY_ARRAY (not with FDTD_KERNEL_FUSED)          */
+  int32_t density;        /* FDTD_DENSITY_UNIFORM / FDTD_DENSITY_ARRAY                                       */
+  int32_t medium;         /* FDTD_MEDIUM_ARRAY (default) / FDTD_MEDIUM_UNIFORM                               */
   int32_t device;         /* CUDA device ordinal                                                             */
   void* stream;           /* cudaStream_t the work is enqueued on (0 = legacy default stream)                */
   void* workspace;        /* DEVICE memory, 256-byte aligned, owned by the caller, must outlive the context  */
@@ -78,7 +85,8 @@ typedef struct {
 } fdtd_params;
 
 /* Bytes of device workspace fdtd_create needs for these parameters (fields p, vx, vy, vz, the per-node
- * K dt/dx array, slab-local psi arrays, CPML tables, source tables, halo buffers).  0 on invalid parameters.
+ * K dt/dx array unless params.medium = FDTD_MEDIUM_UNIFORM, slab-local psi arrays, CPML tables, source tables;
+ * FDTD_KERNEL_FUSED: a second copy of the fields and psi).  0 on invalid parameters.
  * Reads only the size fields; no CUDA call. */
 uint64_t fdtd_workspace_bytes(const fdtd_params* params);
 
@@ -97,7 +105,8 @@ int fdtd_set_model(fdtd_ctx* ctx, const float* c_host, const float* rho_host);
 
 /* Point sources injected into p (P:193 gives the Ricker shape; R14): after the pressure sub-update of step n,
  * p[ijk_s] += wavelets[s*len + n]; steps n >= len inject nothing.  ijk: HOST, 3*n total-grid indices;
- * wavelets: HOST, n*len fp32.  Copied before return (synchronises the stream).  n = 0 clears the sources. */
+ * wavelets: HOST, n*len fp32.  Copied before return (synchronises the stream).  n = 0 clears the sources.  n counts
+ * every step since fdtd_create, also those taken before this call; sources that share a node are all added, in order. */
 int fdtd_set_sources(fdtd_ctx* ctx, int32_t n, const int32_t* ijk_host, const float* wavelets_host, int32_t len);
 
 /* Advances n time steps: for each step the velocity sub-update v_a -= (dt/rho)[(1/kappa_a) D+_a p + psi_va],
@@ -143,6 +152,12 @@ int fdtd_cpml_table(fdtd_ctx* ctx, int32_t axis, int32_t half, float* a_host, fl
 
 /* The four staggered difference weights c_1..c_4 as the kernels use them (fp32; BASELINE: bit-exact). */
 int fdtd_coeffs(float out_host[4]);
+
+/* The kernel family this context runs: FDTD_KERNEL_AUTO (the TMA-tiled kernels), FDTD_KERNEL_REF or FDTD_KERNEL_FUSED.
+ * A context created with FDTD_KERNEL_AUTO runs the much slower one-thread-per-point FDTD_KERNEL_REF kernels when the
+ * tiled ones do not apply (FDTD_PERIODIC, or a total Nx that is not a multiple of 4: they move whole float4s); this
+ * call is how a caller finds out. */
+int fdtd_kernel_in_use(const fdtd_ctx* ctx);
 
 /* Number of kernel launches (the library's own kernels) enqueued since the context was created. */
 int64_t fdtd_launch_count(const fdtd_ctx* ctx);

@@ -17,13 +17,14 @@ FDTD_PSI_VX, FDTD_PSI_VY, FDTD_PSI_VZ, FDTD_PSI_PX, FDTD_PSI_PY, FDTD_PSI_PZ = r
 FDTD_WALL, FDTD_PERIODIC = 0, 1
 FDTD_KERNEL_AUTO, FDTD_KERNEL_REF, FDTD_KERNEL_FUSED = 0, 1, 2
 FDTD_DENSITY_UNIFORM, FDTD_DENSITY_ARRAY = 0, 1
+FDTD_MEDIUM_ARRAY, FDTD_MEDIUM_UNIFORM = 0, 1
 FDTD_OK, FDTD_EINVAL, FDTD_EWORKSPACE, FDTD_ECUDA, FDTD_EUNSUPPORTED = 0, -1, -2, -3, -4
 
 # every symbol include/fdtd_b200.h declares
 EXPORTS = [
     "fdtd_workspace_bytes", "fdtd_create", "fdtd_set_model", "fdtd_set_sources", "fdtd_step", "fdtd_step_profiled", "fdtd_get_field",
     "fdtd_get_field_box", "fdtd_set_field", "fdtd_fill_hash", "fdtd_get_psi", "fdtd_field_absmax", "fdtd_cpml_table",
-    "fdtd_coeffs", "fdtd_launch_count", "fdtd_dims", "fdtd_destroy", "fdtd_last_error",
+    "fdtd_coeffs", "fdtd_kernel_in_use", "fdtd_launch_count", "fdtd_dims", "fdtd_destroy", "fdtd_last_error",
 ]
 
 
@@ -44,6 +45,7 @@ class fdtd_params(C.Structure):
         ("substeps_per_exchange", C.c_int32),
         ("kernel", C.c_int32),
         ("density", C.c_int32),
+        ("medium", C.c_int32),
         ("device", C.c_int32),
         ("stream", C.c_void_p),
         ("workspace", C.c_void_p),
@@ -80,6 +82,7 @@ def _load():
     L.fdtd_launch_count.restype = C.c_int64
     L.fdtd_launch_count.argtypes = [vp]
     L.fdtd_dims.argtypes = [vp, vp]
+    L.fdtd_kernel_in_use.argtypes = [vp]
     L.fdtd_destroy.argtypes = [vp]
     L.fdtd_last_error.restype = C.c_char_p
     return L
@@ -105,7 +108,7 @@ def fdtd_coeffs():
 
 def make_params(n_interior, cpml=(0,) * 6, dx=1.0, dt=0.4, cpml_order=2, cpml_R0=1e-5, cpml_kappa_max=1.0,
                 cpml_alpha_max=0.0, cpml_c_ref=1.0, boundary=FDTD_WALL, decomp=(1, 1, 1), ghost=0, substeps=0,
-                kernel=FDTD_KERNEL_AUTO, density=FDTD_DENSITY_UNIFORM, device=0):
+                kernel=FDTD_KERNEL_AUTO, density=FDTD_DENSITY_UNIFORM, medium=FDTD_MEDIUM_ARRAY, device=0):
     p = fdtd_params()
     p.n_interior[:] = [int(v) for v in n_interior]
     p.cpml[:] = [int(v) for v in cpml]
@@ -115,7 +118,7 @@ def make_params(n_interior, cpml=(0,) * 6, dx=1.0, dt=0.4, cpml_order=2, cpml_R0
     p.cpml_alpha_max, p.cpml_c_ref = float(cpml_alpha_max), float(cpml_c_ref)
     p.decomp[:] = [int(v) for v in decomp]
     p.ghost, p.substeps_per_exchange = int(ghost), int(substeps)
-    p.kernel, p.density, p.device = int(kernel), int(density), int(device)
+    p.kernel, p.density, p.medium, p.device = int(kernel), int(density), int(medium), int(device)
     return p
 
 
@@ -218,6 +221,9 @@ class Fdtd:
         _check(lib.fdtd_cpml_table(self._h, int(axis), int(half), a.ctypes.data, b.ctypes.data, ik.ctypes.data), "fdtd_cpml_table")
         return a, b, ik
 
+    def kernel_in_use(self):
+        return int(lib.fdtd_kernel_in_use(self._h))
+
     def launch_count(self):
         return int(lib.fdtd_launch_count(self._h))
 
@@ -243,6 +249,7 @@ class Fdtd:
 
 def from_workload(w, **kw):
     """Context + model + sources for an inputs.Workload."""
+    kw.setdefault("medium", FDTD_MEDIUM_ARRAY if w.c is not None else FDTD_MEDIUM_UNIFORM)
     sim = Fdtd(w.n_interior, w.cpml, decomp=kw.pop("decomp", w.decomp), ghost=kw.pop("ghost", w.ghost),
                substeps=kw.pop("substeps", w.substeps), **w.cpml_kwargs(), **kw)
     if w.c is not None:

@@ -10,6 +10,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <string>
+#include <thread>
 #include <algorithm>
 #include <vector>
 
@@ -90,6 +91,7 @@ Geometry make_geometry(const fdtd_params& P) {
   if (P.kernel == FDTD_KERNEL_FUSED && (P.boundary == FDTD_PERIODIC || (n_total_x(P) % 4) != 0))
     return bad("FDTD_KERNEL_FUSED needs WALL boundaries and a total Nx that is a multiple of 4");
   if (P.density != FDTD_DENSITY_UNIFORM && P.density != FDTD_DENSITY_ARRAY) return bad("unknown density selector");
+  if (P.medium != FDTD_MEDIUM_ARRAY && P.medium != FDTD_MEDIUM_UNIFORM) return bad("unknown medium selector");
   if (P.density == FDTD_DENSITY_ARRAY && P.kernel == FDTD_KERNEL_FUSED)
     return bad("FDTD_KERNEL_FUSED is not built for a heterogeneous density (use FDTD_KERNEL_AUTO)");
   if (P.boundary == FDTD_PERIODIC)
@@ -150,8 +152,8 @@ struct Layout {
   std::vector<Dom> doms;
   uint64_t tab[2][3][3];
   int tablen[3];
-  uint64_t step, wav, absmax, halo;
-  uint64_t halo_bytes;
+  uint64_t wav, absmax;
+  bool has_kc = true;
 };
 
 constexpr int MAX_SRC = 64;
@@ -159,6 +161,7 @@ constexpr int MAX_WAV_FLOATS = 1 << 22;
 
 Layout make_layout(const fdtd_params& P, const Geometry& G) {
   Layout L;
+  L.has_kc = P.medium == FDTD_MEDIUM_ARRAY || P.density == FDTD_DENSITY_ARRAY;   // the K dt/dx array is optional (16.4 GB at 1600^3)
   uint64_t off = 0;
   auto take = [&](uint64_t bytes) { uint64_t o = off; off = align_up(off + bytes, 256); return o; };
   for (int cz = 0; cz < G.nd[2]; ++cz)
@@ -183,7 +186,7 @@ Layout make_layout(const fdtd_params& P, const Geometry& G) {
       d.pitch = round_up(d.n[0], 8);
       const uint64_t vol = (uint64_t)d.pitch * d.n[1] * d.n[2] * 4;
       for (int f = 0; f < 4; ++f) d.f[f] = take(vol);
-      d.kc = take(vol);
+      d.kc = L.has_kc ? take(vol) : 0;
       for (int fam = 0; fam < 2; ++fam)
         for (int s = 0; s < 2; ++s) {
           d.psi[fam][0][s] = take((uint64_t)d.ln[0][s] * d.n[1] * d.n[2] * 4 + 16);
@@ -212,20 +215,8 @@ Layout make_layout(const fdtd_params& P, const Geometry& G) {
     for (int fam = 0; fam < 2; ++fam)
       for (int t = 0; t < 3; ++t) L.tab[fam][a][t] = take((uint64_t)L.tablen[a] * 4);
   }
-  L.step = take(64);
   L.absmax = take(64);
   L.wav = take((uint64_t)MAX_WAV_FLOATS * 4);
-  // halo staging: one contiguous send buffer per exchange: the largest face set of 4 fields + psi
-  L.halo_bytes = 0;
-  if (G.nd[1] * G.nd[2] > 1) {
-    uint64_t mx = 0;
-    for (auto& d : L.doms) {
-      const uint64_t fy = (uint64_t)d.n[0] * G.ghost * d.n[2], fz = (uint64_t)d.n[0] * d.n[1] * G.ghost;
-      mx = std::max(mx, std::max(fy, fz));
-    }
-    L.halo_bytes = mx * 4 * 16;   // 4 fields + up to 12 psi pieces, generous
-  }
-  L.halo = take(L.halo_bytes + 16);
   L.total = off;
   return L;
 }
@@ -249,7 +240,7 @@ struct fdtd_ctx {
   bool fused = false;
   int grid_f = 0;
   int nsrc = 0, wlen = 0;
-  long long* d_step;
+  long long step_index = 0;      // time steps taken since fdtd_create (the wavelet index of the next injection, R14)
   float* d_wav;
   int64_t launches = 0;
   int64_t substeps_done = 0;    // sub-updates since the last halo exchange (subdomain mode)
@@ -275,7 +266,6 @@ int plan_launch(fdtd_ctx* c, const void* kernel, int smem, int* grid, int thread
   CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem));
   CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->P.device));
   if (per_sm < 1) { set_err("tiled kernel does not fit on an SM"); return FDTD_ECUDA; }
-  if (const char* e = getenv("FDTD_CTAS_PER_SM")) per_sm = std::max(1, std::min(per_sm, atoi(e)));
   *grid = per_sm * sms;
   return FDTD_OK;
 }
@@ -289,7 +279,6 @@ void plan_items(Domain& d, int grid) {
   // about 8 items per resident CTA, chunks of 16..64 planes (each chunk re-reads 7 planes of the z-halo operand)
   long long zc = (long long)v.nz * tiles / (8LL * std::max(grid, 1));
   zc = std::max(16LL, std::min(64LL, zc));
-  if (const char* e = getenv("FDTD_ZCHUNK")) zc = std::max(1, atoi(e));
   int n = (int)((v.nz + zc - 1) / zc);
   S.zchunk = (v.nz + n - 1) / n;
   S.nzc = (v.nz + S.zchunk - 1) / S.zchunk;
@@ -308,16 +297,14 @@ void plan_items_fused(Domain& d, int grid, std::vector<int4>& table) {
   const long long tiles = (long long)S.ntx * S.nty;
   long long zc = (long long)v.nz * tiles / (12LL * std::max(grid, 1));
   zc = std::max(32LL, std::min(256LL, zc));
-  bool uniform = false;
-  if (const char* e = getenv("FDTD_ZCHUNK_FUSED")) { zc = std::max(1, atoi(e)); uniform = true; }
   // z-chunk boundaries: the first rounds take 1.5 zc planes, later ones shrink towards 32
   std::vector<int> zb{0};
-  double sz = uniform ? (double)zc : 1.5 * (double)zc;
+  double sz = 1.5 * (double)zc;
   while (zb.back() < v.nz) {
-    int take = (int)std::max(uniform ? 1.0 : 32.0, sz);
+    int take = (int)std::max(32.0, sz);
     if (v.nz - zb.back() - take < 24) take = v.nz - zb.back();          // no tiny last chunk: every chunk pays a 14-plane lead-in
     zb.push_back(std::min(v.nz, zb.back() + take));
-    if (!uniform) sz *= 0.8;
+    sz *= 0.8;
   }
   auto touches_slab = [&](int axis, int lo, int hi) {
     return (v.ln[axis][0] > 0 && lo < v.ls[axis][0] + v.ln[axis][0] && hi > v.ls[axis][0]) ||
@@ -332,7 +319,7 @@ void plan_items_fused(Domain& d, int grid, std::vector<int4>& table) {
         const bool slab = touches_slab(0, x0, x0 + TX) || touches_slab(1, y0, y0 + TY);
         items.push_back({(zb[c + 1] - zb[c] + 4) * (slab ? 1.5 : 1.0), make_int4(x0, y0, zb[c], zb[c + 1])});
       }
-  if (!uniform) std::stable_sort(items.begin(), items.end(), [](const Item& a, const Item& b) { return a.cost > b.cost; });
+  std::stable_sort(items.begin(), items.end(), [](const Item& a, const Item& b) { return a.cost > b.cost; });
   table.clear();
   for (auto& it : items) table.push_back(it.t);
   S.zchunk = (int)zc;
@@ -376,11 +363,13 @@ int launch_substep(fdtd_ctx* c, Domain& d, int which /*0 = v, 1 = p*/) {
   return FDTD_OK;
 }
 
+// Source injection of time step number c->step_index (R14), then the step index advances — with or without sources.
 int launch_inject(fdtd_ctx* c) {
-  if (c->nsrc == 0) return FDTD_OK;   // the step counter only matters to the wavelet index
+  const long long n = c->step_index++;
+  if (c->nsrc == 0 || n >= c->wlen) return FDTD_OK;
   for (size_t k = 0; k < c->doms.size(); ++k) {
-    SourceView S{c->nsrc, c->wlen, c->doms[k].src_offset, c->doms[k].v.f[0], c->d_wav, c->d_step};
-    inject_sources<<<1, 64, 0, c->stream>>>(S, k + 1 == c->doms.size());
+    SourceView S{c->nsrc, c->wlen, c->doms[k].src_offset, c->doms[k].v.f[0], c->d_wav};
+    inject_sources<<<1, 64, 0, c->stream>>>(S, n);
     c->launches++;
   }
   CK(cudaGetLastError());
@@ -531,6 +520,22 @@ int do_substep(fdtd_ctx* c, int which) {
   return FDTD_OK;
 }
 
+// every value > 0 and finite (NaN fails the first test); split over a few host threads: 4e9 values at config 4
+bool all_positive_finite(const float* a, size_t n) {
+  const unsigned nt = (unsigned)std::max<size_t>(1, std::min<size_t>(std::min<size_t>(16, std::thread::hardware_concurrency()), n >> 20));
+  std::vector<char> ok(nt, 1);
+  std::vector<std::thread> th;
+  for (unsigned t = 0; t < nt; ++t)
+    th.emplace_back([&, t] {
+      const size_t lo = n * t / nt, hi = n * (t + 1) / nt;
+      bool good = true;
+      for (size_t q = lo; q < hi; ++q) good = good && (a[q] > 0.0f) && (a[q] <= 3.0e38f);
+      ok[t] = good;
+    });
+  for (auto& x : th) x.join();
+  return std::all_of(ok.begin(), ok.end(), [](char v) { return v != 0; });
+}
+
 // gather / scatter between a packed host total-grid array and the domains
 int copy_field(fdtd_ctx* c, float* const* dom_base, float* host, bool to_host, bool owned_only) {
   const int gnx = c->G.gn[0], gny = c->G.gn[1];
@@ -620,7 +625,6 @@ fdtd_ctx* fdtd_create(const fdtd_params* P) {
     }
   if ((e = cudaStreamSynchronize(c->stream)) != cudaSuccess) return fail(c, e, "cudaStreamSynchronize");
 
-  c->d_step = (long long*)(c->ws + L.step);
   c->d_wav = (float*)(c->ws + L.wav);
 
   EncodeTiledFn enc = nullptr;
@@ -665,7 +669,7 @@ fdtd_ctx* fdtd_create(const fdtd_params* P) {
       d.src_offset = (long long*)(c->ws + ld.src_off);
       d.counters = (unsigned int*)(c->ws + ld.counters);
       if (!c->use_ref) {
-        float* kcbase = (float*)(c->ws + ld.kc);
+        float* kcbase = L.has_kc ? (float*)(c->ws + ld.kc) : (float*)(c->ws + ld.f[0]);   // no Kc slot: the map is never used
         auto make_maps = [&](TMaps& tm, float* const f[4]) -> int {
           float* tile_base[5] = {f[0], f[1], f[2], f[3], kcbase};
           int bad = make_tmap(enc, &tm.p_halo, f[0], v, HW, VH) || make_tmap(enc, &tm.vx_halo, f[1], v, HW, TY) ||
@@ -779,8 +783,14 @@ int fdtd_set_model(fdtd_ctx* c, const float* c_host, const float* rho_host) {
     bool uniform = true;
     for (size_t q = 1; q < n && uniform; ++q) uniform = rho_host[q] == rho_host[0];
     if (!uniform) return set_model_density_array(c, c_host, rho_host);
-    if (!(rho > 0.0)) { set_err("rho must be positive"); return FDTD_EINVAL; }
+    if (!(rho > 0.0) || rho > 1e30) { set_err("rho must be positive and finite"); return FDTD_EINVAL; }
   }
+  // validate before anything is touched, so that an error leaves the context as it was
+  if (c_host && !c->L.has_kc) {
+    set_err("a wave-speed array needs params.medium = FDTD_MEDIUM_ARRAY (this workspace was sized without the K dt/dx array)");
+    return FDTD_EUNSUPPORTED;
+  }
+  if (c_host && !all_positive_finite(c_host, n)) { set_err("c must be positive and finite"); return FDTD_EINVAL; }
   for (auto& d : c->doms)
     for (int a = 0; a < 3; ++a) d.v.bq[a] = nullptr;
   const float b0 = (float)(c->P.dt / (rho * c->P.dx));
@@ -793,18 +803,13 @@ int fdtd_set_model(fdtd_ctx* c, const float* c_host, const float* rho_host) {
   for (size_t k = 0; k < c->doms.size(); ++k) bases.push_back((float*)(c->ws + c->L.doms[k].kc));
   int r = copy_field(c, bases.data(), const_cast<float*>(c_host), false, false);
   if (r) return r;
-  int* bad = (int*)(c->ws + c->L.absmax) + 4;
-  CK(cudaMemsetAsync(bad, 0, 4, c->stream));
   for (size_t k = 0; k < c->doms.size(); ++k) {
     const DomainView& v = c->doms[k].v;
-    speed_to_kc_kernel<<<148 * 8, 256, 0, c->stream>>>(bases[k], (long long)v.plane * v.nz, v.pitch, v.nx, rho, c->P.dt, c->P.dx, bad);
+    speed_to_kc_kernel<<<148 * 8, 256, 0, c->stream>>>(bases[k], (long long)v.plane * v.nz, v.pitch, v.nx, rho, c->P.dt, c->P.dx);
     c->launches++;
   }
   CK(cudaGetLastError());
-  int nbad = 0;
-  CK(cudaMemcpyAsync(&nbad, bad, 4, cudaMemcpyDeviceToHost, c->stream));
   CK(cudaStreamSynchronize(c->stream));
-  if (nbad) { set_err("c must be positive and finite"); return FDTD_EINVAL; }
   for (size_t k = 0; k < c->doms.size(); ++k) { c->doms[k].v.kc = bases[k]; c->doms[k].v.b0 = b0; }
   return FDTD_OK;
 }
@@ -850,50 +855,58 @@ int fdtd_step(fdtd_ctx* c, int32_t n) {
 int fdtd_step_profiled(fdtd_ctx* c, int32_t n, double out_ms[4]) {
   if (!c || n < 0 || !out_ms) return FDTD_EINVAL;
   // One CUDA event on the launching stream after every launch group; the interval that ends at a mark is
-  // charged to the mark's category (0 = update_v, 1 = update_p, 2 = inject, 3 = exchange).
-  std::vector<cudaEvent_t> ev;
-  std::vector<int> cat;
+  // charged to the mark's category (0 = update_v / step_fused, 1 = update_p, 2 = inject, 3 = exchange).  The events are
+  // created up front and destroyed on every way out.
+  std::vector<cudaEvent_t> ev((size_t)n * 5 + 1, nullptr);
+  std::vector<int> cat(ev.size(), -1);
+  size_t used = 0;
   int r = FDTD_OK;
-  auto mark = [&](int category) -> int {
-    cudaEvent_t e;
-    CK(cudaEventCreate(&e));
-    CK(cudaEventRecord(e, c->stream));
-    ev.push_back(e); cat.push_back(category);
-    return FDTD_OK;
+  cudaError_t ce = cudaSuccess;
+  for (auto& e : ev)
+    if (ce == cudaSuccess) ce = cudaEventCreate(&e);
+  auto mark = [&](int category) {
+    if (ce == cudaSuccess) ce = cudaEventRecord(ev[used], c->stream);
+    cat[used++] = category;
   };
-  r = mark(-1);
-  for (int s = 0; s < n && !r; ++s) {
+  if (ce == cudaSuccess) mark(-1);
+  for (int s = 0; s < n && !r && ce == cudaSuccess; ++s) {
     if (c->fused) {
       if (c->doms.size() > 1 && c->substeps_done % c->G.msub == 0) {
         r = exchange_halos(c);
-        if (!r) r = mark(3);
+        mark(3);
       }
       for (auto& d : c->doms) if (!r) r = launch_fused(c, d);
       c->substeps_done += 2;
-      if (!r) r = mark(0);
+      mark(0);
     }
     for (int which = 0; which < 2 && !r && !c->fused; ++which) {
       if (c->doms.size() > 1 && c->substeps_done % c->G.msub == 0) {
         r = exchange_halos(c);
-        if (!r) r = mark(3);
+        mark(3);
       }
       for (auto& d : c->doms) if (!r) r = launch_substep(c, d, which);
       c->substeps_done++;
-      if (!r) r = mark(which);
+      mark(which);
     }
-    if (!r && c->nsrc > 0) { r = launch_inject(c); if (!r) r = mark(2); }
+    if (!r) { const int64_t l0 = c->launches; r = launch_inject(c); if (c->launches > l0) mark(2); }
   }
-  cudaError_t se = cudaStreamSynchronize(c->stream);
+  if (ce == cudaSuccess) ce = cudaStreamSynchronize(c->stream);
   out_ms[0] = out_ms[1] = out_ms[2] = out_ms[3] = 0.0;
-  if (!r && se == cudaSuccess)
-    for (size_t k = 1; k < ev.size(); ++k) {
+  if (!r && ce == cudaSuccess)
+    for (size_t k = 1; k < used; ++k) {
       float ms = 0.f;
       cudaEventElapsedTime(&ms, ev[k - 1], ev[k]);
       out_ms[cat[k]] += ms;
     }
-  for (auto& e : ev) cudaEventDestroy(e);
-  CK(se);
+  for (auto& e : ev)
+    if (e) cudaEventDestroy(e);
+  CK(ce);
   return r;
+}
+
+int fdtd_kernel_in_use(const fdtd_ctx* c) {
+  if (!c) return FDTD_EINVAL;
+  return c->fused ? FDTD_KERNEL_FUSED : (c->use_ref ? FDTD_KERNEL_REF : FDTD_KERNEL_AUTO);
 }
 
 static int field_bases(fdtd_ctx* c, int which, std::vector<float*>& bases) {

@@ -646,29 +646,35 @@ __global__ void __launch_bounds__(NT, 2) update_p_tiled(const __grid_constant__ 
 
 
 // ---------------------------------------------------------------- small kernels
-// p[src_s] += w_s[n] for every source, then n <- n + 1 (R14).  One block; the step counter lives on the device so
-// that a time step is a fixed launch sequence.
+// p[src_s] += w_s[n] for every source (R14).  The step index n is kept on the host and passed in, so steps taken
+// before fdtd_set_sources count too.  Sources that share a node are added by the first of them, one after the other in
+// source order — the order of the recurrence (oracle: a plain loop over the sources), and no lost update.
 struct SourceView {
   int n, len;
   const long long* offset;   // flat element offset of each source in its domain's p array, or -1 if not held
   float* p;
   const float* wav;
-  long long* step;           // device step counter (shared by all domains; advanced by the launch with advance = 1)
 };
-__global__ void inject_sources(SourceView S, int advance) {
-  const long long n = *S.step;
-  __syncthreads();
-  for (int s = threadIdx.x; s < S.n; s += blockDim.x)
-    if (n < S.len && S.offset[s] >= 0) S.p[S.offset[s]] = __fadd_rn(S.p[S.offset[s]], S.wav[(long long)s * S.len + n]);
-  if (advance && threadIdx.x == 0) *S.step = n + 1;
+__global__ void inject_sources(SourceView S, long long n) {
+  if (n >= S.len) return;
+  for (int s = threadIdx.x; s < S.n; s += blockDim.x) {
+    const long long off = S.offset[s];
+    if (off < 0) continue;
+    bool first = true;
+    for (int t = 0; t < s; ++t) first = first && S.offset[t] != off;
+    if (!first) continue;
+    float v = S.p[off];
+    for (int t = s; t < S.n; ++t)
+      if (S.offset[t] == off) v = __fadd_rn(v, S.wav[(long long)t * S.len + n]);
+    S.p[off] = v;
+  }
 }
 
 // In place: wave speed c (fp32) -> K dt/dx = rho c^2 dt/dx in double, rounded once to fp32 (R6).  Padding columns stay 0.
-__global__ void speed_to_kc_kernel(float* a, long long n, int pitch, int nx, double rho, double dt, double dx, int* bad) {
+__global__ void speed_to_kc_kernel(float* a, long long n, int pitch, int nx, double rho, double dt, double dx) {
   for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
     if ((int)(t % pitch) >= nx) { a[t] = 0.f; continue; }
     const double c = (double)a[t];
-    if (!(c > 0.0) || c > 1e30) atomicAdd(bad, 1);
     a[t] = (float)(rho * c * c * dt / dx);
   }
 }

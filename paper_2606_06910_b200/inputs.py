@@ -7,6 +7,7 @@ once on the host and handed as the same fp32 arrays to both sides (DESIGN.md
 "Input recipe").  The paper uses no dataset (homogeneous cubes with CPML,
 PAPER.md P:290-303); these configs stand in for its workloads at B200 scale.
 """
+import functools
 import math
 
 import numpy as np
@@ -64,10 +65,11 @@ def normals(seed, count, start=0):
     return np.sqrt(-2.0 * np.log(1.0 - u1)) * np.cos(2.0 * math.pi * u2)
 
 
+@functools.lru_cache(maxsize=2)
 def smooth_medium(shape_xyz, seed=20260691, sigma=8.0, amp=0.3, lo=0.7, hi=1.3):
     """Heterogeneous wave speed of BASELINE config 3 (reading R22): seeded N(0,1) field, separable
     Gaussian filter (sigma cells, truncated at 4 sigma, periodic wrap), re-normalised to zero mean /
-    unit std, c = clip(1 + amp g, lo, hi).  Returns fp32 (Nz,Ny,Nx)."""
+    unit std, c = clip(1 + amp g, lo, hi).  Returns fp32 (Nz,Ny,Nx), read-only (cached: half a minute at 552^3)."""
     from scipy.ndimage import gaussian_filter1d
 
     nx, ny, nz = shape_xyz
@@ -83,6 +85,7 @@ def smooth_medium(shape_xyz, seed=20260691, sigma=8.0, amp=0.3, lo=0.7, hi=1.3):
     g *= np.float32(1.0 / s)
     c = np.float32(1.0) + np.float32(amp) * g
     np.clip(c, lo, hi, out=c)
+    c.setflags(write=False)
     return c
 
 

@@ -323,3 +323,79 @@ def test_errors_are_reported_not_fatal(B):
     for bad in (dict(n_interior=(18, 16, 16)), dict(n_interior=(16,) * 3, boundary=B.FDTD_PERIODIC)):
         with pytest.raises(B.FdtdError):                            # the fused step refuses what it cannot run
             B.Fdtd(bad.pop("n_interior"), dt=0.4, kernel=B.FDTD_KERNEL_FUSED, **bad)
+
+
+@pytest.mark.parametrize("kernel", [1, 0, 2])
+def test_sources_sharing_a_node_and_steps_before_set_sources(B, kernel):
+    """R14: the wavelet index is the time-step number since creation, also for steps taken before fdtd_set_sources;
+    three sources on one node are all added, in source order, as the oracle's plain loop does (bit for bit: a
+    homogeneous run from zero fields with one active node goes through the same additions on both sides)."""
+    shape, steps = (24, 20, 28), 9
+    src = np.array([[12, 10, 14], [5, 6, 7], [12, 10, 14], [12, 10, 14]], np.int32)
+    wav = np.stack([inputs.ricker(steps, 0.4, t0=2.0), 0.3 * inputs.ricker(steps, 0.4, t0=1.0),
+                    np.full(steps, 1e-3, np.float32), np.linspace(-1, 1, steps).astype(np.float32)])
+    sim = B.Fdtd(shape, dt=0.4, kernel=kernel)
+    o = Oracle(shape, dt=0.4)
+    sim.step(3)                                  # nothing to inject yet, but the steps count
+    o.step(3)
+    sim.set_sources(src, wav)
+    o.set_sources(src, wav)
+    sim.step(1)
+    o.step(1)
+    p = sim.get_field(B.FDTD_P)
+    assert p[14, 10, 12] == np.float32(np.float32(np.float32(wav[0, 3]) + wav[2, 3]) + wav[3, 3])
+    assert p[7, 6, 5] == wav[1, 3]
+    sim.step(steps - 4)
+    o.step(steps - 4)
+    for f in range(4):
+        assert rel(sim.get_field(f), o.get(f)) <= TOL, f
+    sim.step(3)                                  # past the end of the table: nothing is injected, nothing breaks
+    o.step(3)
+    assert rel(sim.get_field(0), o.get(0)) <= TOL
+    sim.destroy()
+
+
+def test_invalid_model_leaves_the_context_unchanged(B):
+    """Header contract: on error the context is left unchanged — a rejected c must not clobber the installed K dt/dx."""
+    shape = (40, 24, 24)
+    rng = np.random.default_rng(5)
+    c = (1.0 + 0.3 * rng.random(shape[::-1])).astype(np.float32)
+    runs = []
+    for poison in (False, True):
+        sim = B.Fdtd(shape, dt=0.3)
+        sim.set_model(c)
+        if poison:
+            bad = c.copy()
+            bad[3, 4, 5] = -1.0
+            with pytest.raises(B.FdtdError):
+                sim.set_model(bad)
+            bad[3, 4, 5] = np.nan
+            with pytest.raises(B.FdtdError):
+                sim.set_model(bad)
+        for f in range(4):
+            sim.fill_hash(f, 8, 0.5)
+        sim.step(4)
+        runs.append([sim.get_field(f) for f in range(4)])
+        sim.destroy()
+    for a, b in zip(*runs):
+        assert np.array_equal(a, b)
+
+
+def test_kernel_in_use_reports_the_reference_fallback_and_uniform_medium_refuses_an_array(B):
+    sim = B.Fdtd((64, 16, 16), dt=0.4)
+    assert sim.kernel_in_use() == B.FDTD_KERNEL_AUTO
+    sim.destroy()
+    sim = B.Fdtd((66, 16, 16), dt=0.4)                         # Nx % 4 != 0: AUTO falls back, and says so
+    assert sim.kernel_in_use() == B.FDTD_KERNEL_REF
+    sim.destroy()
+    sim = B.Fdtd((64, 16, 16), dt=0.4, kernel=B.FDTD_KERNEL_FUSED, medium=B.FDTD_MEDIUM_UNIFORM)
+    assert sim.kernel_in_use() == B.FDTD_KERNEL_FUSED
+    small = sim.workspace_bytes
+    with pytest.raises(B.FdtdError):
+        sim.set_model(np.ones(sim.shape, np.float32))
+    sim.set_model(None)
+    sim.step(2)
+    sim.destroy()
+    sim = B.Fdtd((64, 16, 16), dt=0.4, kernel=B.FDTD_KERNEL_FUSED)
+    assert sim.workspace_bytes >= small + 64 * 16 * 16 * 4
+    sim.destroy()

@@ -101,19 +101,27 @@ def test_other_layouts_slab_and_more_subdomains(B):
             assert _same_bits(a, b), decomp
 
 
-@pytest.mark.parametrize("kernel", [0, 2])
-def test_config5_full_size_bit_identical(B, kernel):
-    """The full BASELINE config 5: 512^3 + 20-cell CPML as 1x2x2, centre source on the 4-subdomain corner, 400 steps,
-    (g, m) = (8, 2) — the paper's s = 1 — compared with the monolithic two-kernel run on all four fields; the subdomains
-    run the two-kernel step (kernel 0) or the single-pass step (kernel 2)."""
+@pytest.fixture(scope="module")
+def config5_monolithic(B):
+    """The monolithic two-kernel run of BASELINE config 5 (552^3, centre source, 400 steps): the four final fields."""
     w = inputs.config(5)
     mono = B.from_workload(w, decomp=(1, 1, 1), ghost=0, substeps=0)
     mono.step(w.steps)
-    sub = B.from_workload(w, decomp=(1, 2, 2), ghost=8, substeps=2, kernel=kernel)
+    out = [mono.get_field(f) for f in range(4)]
+    mono.destroy()
+    assert all(np.abs(a).max() > 0 for a in out)
+    return out
+
+
+@pytest.mark.parametrize("g,m,kernel", [(4, 1, 0), (8, 2, 0), (8, 2, 2), (16, 4, 0), (16, 4, 2), (32, 8, 2)])
+def test_config5_full_size_bit_identical(B, config5_monolithic, g, m, kernel):
+    """The full BASELINE config 5: 512^3 + 20-cell CPML as 1x2x2, centre source on the 4-subdomain corner, 400 steps, at
+    every (g, m) BASELINE names — g = 4k for k = 1, 2, 4 sub-updates per exchange (R20) — and at the paper's s = 4
+    (g = 32): all four fields have the bits of the monolithic two-kernel run.  The subdomains run the two-kernel
+    step (kernel 0) or the single-pass step (kernel 2, which advances two sub-updates per launch, so m is even)."""
+    w = inputs.config(5)
+    sub = B.from_workload(w, decomp=(1, 2, 2), ghost=g, substeps=m, kernel=kernel)
     sub.step(w.steps)
     for f in range(4):
-        a, b = mono.get_field(f), sub.get_field(f)
-        assert np.abs(a).max() > 0
-        assert _same_bits(a, b), f
-    mono.destroy()
+        assert _same_bits(config5_monolithic[f], sub.get_field(f)), (g, m, kernel, f)
     sub.destroy()
