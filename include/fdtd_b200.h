@@ -51,6 +51,12 @@ enum {
                           /* fdtd_set_model with a c array then returns FDTD_EUNSUPPORTED                                */
 };
 enum {
+  FDTD_PRECISION_FP32 = 0, /* single precision state and arithmetic: the product path                     */
+  FDTD_PRECISION_FP64 = 1  /* "verification precision": fields, memory variables and arithmetic in double; every */
+                           /* coefficient stays the fp32 number of the fp32 path.  One-thread-per-point kernels only,    */
+                           /* monolithic only; fields move through the *_f64 entry points                                */
+};
+enum {
   FDTD_KERNEL_AUTO = 0, /* TMA-staged, z-streaming tile kernels (the product path)                        */
   FDTD_KERNEL_REF = 1,  /* one thread per point, global loads only; also the only path for FDTD_PERIODIC   */
   FDTD_KERNEL_FUSED = 2 /* one launch per time step: both sub-updates in a single pass over the fields (32 B  */
@@ -71,13 +77,15 @@ typedef struct {
   double cpml_kappa_max;  /* kappa_max                                                        */
   double cpml_alpha_max;  /* alpha_max                                                        */
   double cpml_c_ref;      /* wave speed absorbed into sigma_max = -(q+1) c_ref ln(R0) / (2 L dx) (R7)        */
-  int32_t decomp[3];      /* in-HBM subdomain grid; {1,1,1} (or zeros) = monolithic.  decomp[0] must be 1:   */
-                          /* pencil-yz keeps x local                                                  */
+  int32_t decomp[3];      /* in-HBM subdomain grid Px, Py, Pz; {1,1,1} (or zeros) = monolithic.  1 x Py x Pz is */
+                          /* the paper's pencil-yz (x stays local and contiguous), 1 x 1 x Pz slab-z,     */
+                          /* Px x Py x 1 block-xy; an x cut needs widths and ghost that are multiples of 4      */
   int32_t ghost;          /* ghost depth g in cells on every internal interface                 */
   int32_t substeps_per_exchange; /* m sub-updates (v or p) between halo exchanges; needs g >= 4 m (R20)      */
   int32_t kernel;         /* FDTD_KERNEL_AUTO / FDTD_KERNEL_REF / FDTD_KERNEL_FUSED                          */
   int32_t density;        /* FDTD_DENSITY_UNIFORM / FDTD_DENSITY_ARRAY                                       */
   int32_t medium;         /* FDTD_MEDIUM_ARRAY (default) / FDTD_MEDIUM_UNIFORM                               */
+  int32_t precision;      /* FDTD_PRECISION_FP32 (default) / FDTD_PRECISION_FP64                             */
   int32_t device;         /* CUDA device ordinal                                                             */
   void* stream;           /* cudaStream_t the work is enqueued on (0 = legacy default stream)                */
   void* workspace;        /* DEVICE memory, 256-byte aligned, owned by the caller, must outlive the context  */
@@ -126,6 +134,11 @@ int fdtd_step_profiled(fdtd_ctx* ctx, int32_t n, double out_ms_host[4]);
  * mode the owned cells of every subdomain are gathered.  Synchronises the stream. */
 int fdtd_get_field(fdtd_ctx* ctx, int32_t which, float* dst_host);
 
+/* The same two calls for a context created with FDTD_PRECISION_FP64 (Nz*Ny*Nx doubles).  The fp32 calls refuse an fp64
+ * context and the other way round (FDTD_EUNSUPPORTED). */
+int fdtd_get_field_f64(fdtd_ctx* ctx, int32_t which, double* dst_host);
+int fdtd_set_field_f64(fdtd_ctx* ctx, int32_t which, const double* src_host);
+
 /* Sub-box [lo, lo+size) of one field to dst_host (size[2]*size[1]*size[0] fp32, x fastest).  Synchronises. */
 int fdtd_get_field_box(fdtd_ctx* ctx, int32_t which, const int32_t lo[3], const int32_t size[3], float* dst_host);
 
@@ -141,6 +154,8 @@ int fdtd_fill_hash(fdtd_ctx* ctx, int32_t which, uint64_t seed, double scale);
 /* One CPML memory variable (FDTD_PSI_*) expanded from its slab-local storage to the full total grid (zeros
  * outside the slabs) into dst_host — debugging / parity of the recursion.  Synchronises. */
 int fdtd_get_psi(fdtd_ctx* ctx, int32_t which, float* dst_host);
+
+int fdtd_get_psi_f64(fdtd_ctx* ctx, int32_t which, double* dst_host);   /* the same for an fp64 context */
 
 /* max |f| over the box [lo, lo+size) of one field, reduced on the device; result to *out_host.  Synchronises. */
 int fdtd_field_absmax(fdtd_ctx* ctx, int32_t which, const int32_t lo[3], const int32_t size[3], float* out_host);

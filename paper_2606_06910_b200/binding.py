@@ -18,12 +18,13 @@ FDTD_WALL, FDTD_PERIODIC = 0, 1
 FDTD_KERNEL_AUTO, FDTD_KERNEL_REF, FDTD_KERNEL_FUSED = 0, 1, 2
 FDTD_DENSITY_UNIFORM, FDTD_DENSITY_ARRAY = 0, 1
 FDTD_MEDIUM_ARRAY, FDTD_MEDIUM_UNIFORM = 0, 1
+FDTD_PRECISION_FP32, FDTD_PRECISION_FP64 = 0, 1
 FDTD_OK, FDTD_EINVAL, FDTD_EWORKSPACE, FDTD_ECUDA, FDTD_EUNSUPPORTED = 0, -1, -2, -3, -4
 
 # every symbol include/fdtd_b200.h declares
 EXPORTS = [
     "fdtd_workspace_bytes", "fdtd_create", "fdtd_set_model", "fdtd_set_sources", "fdtd_step", "fdtd_step_profiled", "fdtd_get_field",
-    "fdtd_get_field_box", "fdtd_set_field", "fdtd_fill_hash", "fdtd_get_psi", "fdtd_field_absmax", "fdtd_cpml_table",
+    "fdtd_get_field_box", "fdtd_set_field", "fdtd_get_field_f64", "fdtd_set_field_f64", "fdtd_get_psi_f64", "fdtd_fill_hash", "fdtd_get_psi", "fdtd_field_absmax", "fdtd_cpml_table",
     "fdtd_coeffs", "fdtd_kernel_in_use", "fdtd_launch_count", "fdtd_dims", "fdtd_destroy", "fdtd_last_error",
 ]
 
@@ -46,6 +47,7 @@ class fdtd_params(C.Structure):
         ("kernel", C.c_int32),
         ("density", C.c_int32),
         ("medium", C.c_int32),
+        ("precision", C.c_int32),
         ("device", C.c_int32),
         ("stream", C.c_void_p),
         ("workspace", C.c_void_p),
@@ -74,6 +76,9 @@ def _load():
     L.fdtd_get_field.argtypes = [vp, i32, vp]
     L.fdtd_get_field_box.argtypes = [vp, i32, vp, vp, vp]
     L.fdtd_set_field.argtypes = [vp, i32, vp]
+    L.fdtd_get_field_f64.argtypes = [vp, i32, vp]
+    L.fdtd_set_field_f64.argtypes = [vp, i32, vp]
+    L.fdtd_get_psi_f64.argtypes = [vp, i32, vp]
     L.fdtd_fill_hash.argtypes = [vp, i32, u64, f64]
     L.fdtd_get_psi.argtypes = [vp, i32, vp]
     L.fdtd_field_absmax.argtypes = [vp, i32, vp, vp, vp]
@@ -108,7 +113,7 @@ def fdtd_coeffs():
 
 def make_params(n_interior, cpml=(0,) * 6, dx=1.0, dt=0.4, cpml_order=2, cpml_R0=1e-5, cpml_kappa_max=1.0,
                 cpml_alpha_max=0.0, cpml_c_ref=1.0, boundary=FDTD_WALL, decomp=(1, 1, 1), ghost=0, substeps=0,
-                kernel=FDTD_KERNEL_AUTO, density=FDTD_DENSITY_UNIFORM, medium=FDTD_MEDIUM_ARRAY, device=0):
+                kernel=FDTD_KERNEL_AUTO, density=FDTD_DENSITY_UNIFORM, medium=FDTD_MEDIUM_ARRAY, precision=FDTD_PRECISION_FP32, device=0):
     p = fdtd_params()
     p.n_interior[:] = [int(v) for v in n_interior]
     p.cpml[:] = [int(v) for v in cpml]
@@ -118,7 +123,7 @@ def make_params(n_interior, cpml=(0,) * 6, dx=1.0, dt=0.4, cpml_order=2, cpml_R0
     p.cpml_alpha_max, p.cpml_c_ref = float(cpml_alpha_max), float(cpml_c_ref)
     p.decomp[:] = [int(v) for v in decomp]
     p.ghost, p.substeps_per_exchange = int(ghost), int(substeps)
-    p.kernel, p.density, p.medium, p.device = int(kernel), int(density), int(medium), int(device)
+    p.kernel, p.density, p.medium, p.precision, p.device = int(kernel), int(density), int(medium), int(precision), int(device)
     return p
 
 
@@ -176,7 +181,16 @@ class Fdtd:
         _check(lib.fdtd_step_profiled(self._h, int(n), out.ctypes.data), "fdtd_step_profiled")
         return dict(update_v=float(out[0]), update_p=float(out[1]), inject=float(out[2]), exchange=float(out[3]))
 
+    @property
+    def fp64(self):
+        return self.params.precision == FDTD_PRECISION_FP64
+
     def get_field(self, which, out=None):
+        """float32 array, or float64 for a context created with precision=FDTD_PRECISION_FP64."""
+        if self.fp64:
+            out = np.empty(self.shape, np.float64) if out is None else out
+            _check(lib.fdtd_get_field_f64(self._h, int(which), out.ctypes.data), "fdtd_get_field_f64")
+            return out
         if out is None:
             out = np.empty(self.shape, np.float32)
         _check(lib.fdtd_get_field(self._h, int(which), out.ctypes.data), "fdtd_get_field")
@@ -197,6 +211,10 @@ class Fdtd:
         return out
 
     def set_field(self, which, arr):
+        if self.fp64:
+            a = np.ascontiguousarray(arr, np.float64).reshape(self.shape)
+            _check(lib.fdtd_set_field_f64(self._h, int(which), a.ctypes.data), "fdtd_set_field_f64")
+            return
         a = np.ascontiguousarray(arr, np.float32).reshape(self.shape)
         _check(lib.fdtd_set_field(self._h, int(which), a.ctypes.data), "fdtd_set_field")
 
@@ -204,6 +222,10 @@ class Fdtd:
         _check(lib.fdtd_fill_hash(self._h, int(which), C.c_uint64(int(seed)), float(scale)), "fdtd_fill_hash")
 
     def get_psi(self, which):
+        if self.fp64:
+            out = np.empty(self.shape, np.float64)
+            _check(lib.fdtd_get_psi_f64(self._h, int(which), out.ctypes.data), "fdtd_get_psi_f64")
+            return out
         out = np.empty(self.shape, np.float32)
         _check(lib.fdtd_get_psi(self._h, int(which), out.ctypes.data), "fdtd_get_psi")
         return out

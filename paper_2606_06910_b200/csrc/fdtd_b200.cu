@@ -92,24 +92,31 @@ Geometry make_geometry(const fdtd_params& P) {
     return bad("FDTD_KERNEL_FUSED needs WALL boundaries and a total Nx that is a multiple of 4");
   if (P.density != FDTD_DENSITY_UNIFORM && P.density != FDTD_DENSITY_ARRAY) return bad("unknown density selector");
   if (P.medium != FDTD_MEDIUM_ARRAY && P.medium != FDTD_MEDIUM_UNIFORM) return bad("unknown medium selector");
-  if (P.density == FDTD_DENSITY_ARRAY && P.kernel == FDTD_KERNEL_FUSED)
-    return bad("FDTD_KERNEL_FUSED is not built for a heterogeneous density (use FDTD_KERNEL_AUTO)");
+  if (P.precision != FDTD_PRECISION_FP32 && P.precision != FDTD_PRECISION_FP64) return bad("unknown precision selector");
+  if (P.precision == FDTD_PRECISION_FP64 && P.kernel == FDTD_KERNEL_FUSED)
+    return bad("the fp64 verification precision runs the one-thread-per-point kernels only (FDTD_KERNEL_AUTO or FDTD_KERNEL_REF)");
   if (P.boundary == FDTD_PERIODIC)
     for (int f = 0; f < 6; ++f) if (P.cpml[f]) return bad("PERIODIC excludes CPML");
   for (int f = 0; f < 6; ++f)
     if (P.cpml[f] > 0 && (!(P.cpml_R0 > 0.0) || P.cpml_order < 1 || !(P.cpml_kappa_max >= 1.0) || P.cpml_alpha_max < 0.0 || !(P.cpml_c_ref > 0.0)))
       return bad("bad CPML parameters");
-  if (G.nd[0] != 1) return bad("decomp[0] must be 1 (pencil-yz keeps x local)");
-  const bool sub = G.nd[1] * G.nd[2] > 1;
+  const bool sub = G.nd[0] * G.nd[1] * G.nd[2] > 1;
+  if (sub && P.precision == FDTD_PRECISION_FP64) return bad("the fp64 verification precision is monolithic only");
   G.ghost = sub ? P.ghost : 0;
   G.msub = sub ? P.substeps_per_exchange : 0;
   if (sub) {
     if (P.boundary == FDTD_PERIODIC) return bad("subdomain mode needs WALL boundaries");
     if (G.msub < 1 || G.ghost < 4 * G.msub) return bad("ghost must be >= 4 * substeps_per_exchange");
     if (P.kernel == FDTD_KERNEL_FUSED && (G.msub % 2)) return bad("the fused step advances two sub-updates: substeps_per_exchange must be even");
-    for (int a = 1; a < 3; ++a) {
+    for (int a = 0; a < 3; ++a) {
       if (G.gn[a] % G.nd[a]) return bad("total grid not divisible by decomp");
       if (G.gn[a] / G.nd[a] < G.ghost) return bad("ghost deeper than a subdomain");
+    }
+    // an x cut (block-xy) keeps every subdomain's rows float4-aligned, and its ghost columns clear of the x layers
+    if (G.nd[0] > 1) {
+      const int own = G.gn[0] / G.nd[0];
+      if ((own % 4) || (G.ghost % 4)) return bad("an x cut needs subdomain widths and a ghost depth that are multiples of 4");
+      if (own - G.ghost < round_up(P.cpml[0], 4) + 4 || own - G.ghost < P.cpml[1] + 8) return bad("an x cut needs subdomains wider than ghost + CPML layer");
     }
   }
   for (int a = 0; a < 3; ++a) {
@@ -127,8 +134,9 @@ Geometry make_geometry(const fdtd_params& P) {
 // One domain on the host: its view plus what the launches need.
 struct Domain {
   DomainView v;
+  DomainViewT<double> v64;     // FDTD_PRECISION_FP64: the same geometry with double fields and psi (v.f / v.psi then alias them)
   int own_lo[3], own_hi[3];    // owned cells in local indices
-  int cy, cz;                  // position in the subdomain grid
+  int cx, cy, cz;              // position in the subdomain grid
   TMaps tm;
   OutSet alt;                  // fused mode: the other state (fields + psi); swapped with v.f / v.psi after every launch
   TMaps tm_alt;                // its tensor maps
@@ -165,9 +173,10 @@ Layout make_layout(const fdtd_params& P, const Geometry& G) {
   uint64_t off = 0;
   auto take = [&](uint64_t bytes) { uint64_t o = off; off = align_up(off + bytes, 256); return o; };
   for (int cz = 0; cz < G.nd[2]; ++cz)
-    for (int cy = 0; cy < G.nd[1]; ++cy) {
+    for (int cy = 0; cy < G.nd[1]; ++cy)
+     for (int cx = 0; cx < G.nd[0]; ++cx) {
       Layout::Dom d{};
-      const int c[3] = {0, cy, cz};
+      const int c[3] = {cx, cy, cz};
       for (int a = 0; a < 3; ++a) {
         const int own = G.gn[a] / G.nd[a];
         const int glo = c[a] > 0 ? G.ghost : 0, ghi = c[a] < G.nd[a] - 1 ? G.ghost : 0;
@@ -184,14 +193,15 @@ Layout make_layout(const fdtd_params& P, const Geometry& G) {
       if (d.ln[0][0] > 0) d.ln[0][0] = round_up(d.ln[0][0], 4);
       if (d.ln[0][1] > 0) d.ln[0][1] = round_up(d.n[0] - d.ls[0][1], 4);
       d.pitch = round_up(d.n[0], 8);
-      const uint64_t vol = (uint64_t)d.pitch * d.n[1] * d.n[2] * 4;
-      for (int f = 0; f < 4; ++f) d.f[f] = take(vol);
+      const uint64_t es = P.precision == FDTD_PRECISION_FP64 ? 8 : 4;          // bytes per field / psi element
+      const uint64_t vol = (uint64_t)d.pitch * d.n[1] * d.n[2] * 4;            // one fp32 array (K dt/dx, dt/(rho_bar dx))
+      for (int f = 0; f < 4; ++f) d.f[f] = take(vol / 4 * es);
       d.kc = L.has_kc ? take(vol) : 0;
       for (int fam = 0; fam < 2; ++fam)
         for (int s = 0; s < 2; ++s) {
-          d.psi[fam][0][s] = take((uint64_t)d.ln[0][s] * d.n[1] * d.n[2] * 4 + 16);
-          d.psi[fam][1][s] = take((uint64_t)d.pitch * d.ln[1][s] * d.n[2] * 4 + 16);
-          d.psi[fam][2][s] = take((uint64_t)d.pitch * d.n[1] * d.ln[2][s] * 4 + 16);
+          d.psi[fam][0][s] = take((uint64_t)d.ln[0][s] * d.n[1] * d.n[2] * es + 16);
+          d.psi[fam][1][s] = take((uint64_t)d.pitch * d.ln[1][s] * d.n[2] * es + 16);
+          d.psi[fam][2][s] = take((uint64_t)d.pitch * d.n[1] * d.ln[2][s] * es + 16);
         }
       if (P.kernel == FDTD_KERNEL_FUSED) {
         d.items_cap = (uint64_t)((d.n[0] + TX - 1) / TX) * ((d.n[1] + TY - 1) / TY) * (d.n[2] / 16 + 8);
@@ -237,6 +247,8 @@ struct fdtd_ctx {
   AxisTable tabs[2][3];
   std::vector<float> dev_a[2][3];
   bool use_ref;
+  bool fp64 = false;
+  size_t es = 4;                // bytes per field / psi element
   bool fused = false;
   int grid_f = 0;
   int nsrc = 0, wlen = 0;
@@ -332,7 +344,8 @@ int launch_fused(fdtd_ctx* c, Domain& d) {
   Sched S = d.sched_f;
   S.counter = d.counters + 2 + d.fused_parity;
   S.other = d.counters + 2 + (1 - d.fused_parity);
-  step_fused<<<std::min(c->grid_f, S.nitems), FNT, F_SMEM_BYTES, c->stream>>>(d.tm, d.v, d.alt, S);
+  if (d.v.bq[0]) step_fused<true><<<std::min(c->grid_f, S.nitems), FNT, f_smem_bytes<true>(), c->stream>>>(d.tm, d.v, d.alt, S);
+  else step_fused<false><<<std::min(c->grid_f, S.nitems), FNT, f_smem_bytes<false>(), c->stream>>>(d.tm, d.v, d.alt, S);
   c->launches++;
   CK(cudaGetLastError());
   d.fused_parity ^= 1;
@@ -348,8 +361,13 @@ int launch_substep(fdtd_ctx* c, Domain& d, int which /*0 = v, 1 = p*/) {
   const DomainView& v = d.v;
   if (c->use_ref) {
     dim3 b(64, 4, 1), g((v.nx + 63) / 64, (v.ny + 3) / 4, v.nz);
-    if (which == 0) update_v_ref<<<g, b, 0, c->stream>>>(v);
-    else update_p_ref<<<g, b, 0, c->stream>>>(v);
+    if (c->fp64) {
+      if (which == 0) update_v_ref<<<g, b, 0, c->stream>>>(d.v64);
+      else update_p_ref<<<g, b, 0, c->stream>>>(d.v64);
+    } else {
+      if (which == 0) update_v_ref<<<g, b, 0, c->stream>>>(v);
+      else update_p_ref<<<g, b, 0, c->stream>>>(v);
+    }
   } else {
     Sched S = d.sched;
     S.counter = d.counters + which;
@@ -368,8 +386,13 @@ int launch_inject(fdtd_ctx* c) {
   const long long n = c->step_index++;
   if (c->nsrc == 0 || n >= c->wlen) return FDTD_OK;
   for (size_t k = 0; k < c->doms.size(); ++k) {
-    SourceView S{c->nsrc, c->wlen, c->doms[k].src_offset, c->doms[k].v.f[0], c->d_wav};
-    inject_sources<<<1, 64, 0, c->stream>>>(S, n);
+    if (c->fp64) {
+      SourceViewT<double> S{c->nsrc, c->wlen, c->doms[k].src_offset, c->doms[k].v64.f[0], c->d_wav};
+      inject_sources<<<1, 64, 0, c->stream>>>(S, n);
+    } else {
+      SourceView S{c->nsrc, c->wlen, c->doms[k].src_offset, c->doms[k].v.f[0], c->d_wav};
+      inject_sources<<<1, 64, 0, c->stream>>>(S, n);
+    }
     c->launches++;
   }
   CK(cudaGetLastError());
@@ -410,35 +433,39 @@ int run_batch(fdtd_ctx* c, const CopyBatch& B) {
   return FDTD_OK;
 }
 
-// Adds the jobs that refresh `dst`'s ghost cells on its low/high side of `axis` (1 = y, 2 = z) from the owner.
-// Phase y copies owned rows over the owned z range only; phase z then copies whole planes (all local rows of the
-// receiving domain, ghost rows included), which carries the corners (R21).
+// Adds the jobs that refresh `dst`'s ghost cells on its low/high side of `axis` (0 = x, 1 = y, 2 = z) from the owner.
+// The phases run x, then y, then z; a phase copies the ghost range along its own axis, the whole local extent (ghost cells
+// included) along the axes already exchanged and the owned range along the axes still to come, which carries the edges and
+// corners (R21).  An x cut moves g-wide column blocks — the strided access that makes block-xy the slow layout.
 void add_face_jobs(fdtd_ctx* c, std::vector<CopyJob>& jobs, Domain& dst, Domain& src, int axis, int side) {
   const DomainView &dv = dst.v, &sv = src.v;
   const int g = c->G.ghost;
-  // destination ghost range along `axis` in dst-local indices, and the same cells in src-local indices
-  const int dlo = side == 0 ? 0 : dst.own_hi[axis];
-  const int glo_global = (axis == 1 ? dv.oy : dv.oz) + dlo;
-  const int slo = glo_global - (axis == 1 ? sv.oy : sv.oz);
-  auto push = [&](const float* sb, float* db, long long sp, long long sr, long long dp, long long dr, int w, int h, int d,
+  const int dn[3] = {dv.nx, dv.ny, dv.nz};
+  const int dofs[3] = {dv.ox, dv.oy, dv.oz}, sofs[3] = {sv.ox, sv.oy, sv.oz};
+  int b0[3], b1[3];                                       // the box in dst-local indices
+  for (int a = 0; a < 3; ++a) {
+    if (a == axis) { b0[a] = side == 0 ? 0 : dst.own_hi[a]; b1[a] = b0[a] + g; }
+    else if (a < axis) { b0[a] = 0; b1[a] = dn[a]; }
+    else { b0[a] = dst.own_lo[a]; b1[a] = dst.own_hi[a]; }
+  }
+  int s0[3];                                              // the same cells in src-local indices
+  for (int a = 0; a < 3; ++a) s0[a] = b0[a] + dofs[a] - sofs[a];
+  const int w = axis == 0 ? g : dv.pitch;                 // phases y, z move whole rows (both pitches are equal)
+  const int dx0 = axis == 0 ? b0[0] : 0, sx0 = axis == 0 ? s0[0] : 0;
+  auto push = [&](const float* sb, float* db, long long sp, long long sr, long long dp, long long dr, int ww, int h, int d,
                   long long soff, long long doff) {
-    if (w <= 0 || h <= 0 || d <= 0) return;
-    jobs.push_back(CopyJob{sb + soff, db + doff, sp, sr, dp, dr, w, h, d});
+    if (ww <= 0 || h <= 0 || d <= 0) return;
+    jobs.push_back(CopyJob{sb + soff, db + doff, sp, sr, dp, dr, ww, h, d});
   };
-  // z range / y range of the box in dst-local and src-local coordinates
-  int dy0, dy1, dz0, dz1;
-  if (axis == 1) { dy0 = dlo; dy1 = dlo + g; dz0 = dst.own_lo[2]; dz1 = dst.own_hi[2]; }
-  else { dy0 = 0; dy1 = dv.ny; dz0 = dlo; dz1 = dlo + g; }
-  const int sy0 = dy0 + dv.oy - sv.oy, sz0 = dz0 + dv.oz - sv.oz;
-  (void)slo;
-  const int w = dv.pitch;   // whole rows: x is never decomposed, both pitches are equal
+  const int dy0 = b0[1], dy1 = b1[1], dz0 = b0[2], dz1 = b1[2], sy0 = s0[1], sz0 = s0[2];
   for (int f = 0; f < 4; ++f)
     push(sv.f[f], dv.f[f], sv.plane, sv.pitch, dv.plane, dv.pitch, w, dy1 - dy0, dz1 - dz0,
-         (long long)sz0 * sv.plane + (long long)sy0 * sv.pitch, (long long)dz0 * dv.plane + (long long)dy0 * dv.pitch);
+         (long long)sz0 * sv.plane + (long long)sy0 * sv.pitch + sx0, (long long)dz0 * dv.plane + (long long)dy0 * dv.pitch + dx0);
   // psi pieces that live in the ghost box (R21): x slabs (all j,k), y slabs (rows in slab), z slabs (planes in slab)
   for (int fam = 0; fam < 2; ++fam) {
     for (int s = 0; s < 2; ++s) {
-      if (dv.ln[0][s] > 0 && sv.ln[0][s] == dv.ln[0][s]) {
+      // x slabs: whole slab width; an x-phase box never meets an x layer (make_geometry)
+      if (axis != 0 && dv.ln[0][s] > 0 && sv.ln[0][s] == dv.ln[0][s]) {
         const int wx = dv.ln[0][s];
         push(sv.psi[fam][0][s], dv.psi[fam][0][s], (long long)sv.ny * wx, wx, (long long)dv.ny * wx, wx, wx, dy1 - dy0, dz1 - dz0,
              ((long long)sz0 * sv.ny + sy0) * wx, ((long long)dz0 * dv.ny + dy0) * wx);
@@ -450,8 +477,8 @@ void add_face_jobs(fdtd_ctx* c, std::vector<CopyJob>& jobs, Domain& dst, Domain&
           const int sa0 = a0 + dv.oy - sv.oy;
           if (sa0 >= sv.ls[1][s] && sa0 + (a1 - a0) <= sv.ls[1][s] + sv.ln[1][s])
             push(sv.psi[fam][1][s], dv.psi[fam][1][s], (long long)sv.ln[1][s] * sv.pitch, sv.pitch, (long long)dv.ln[1][s] * dv.pitch,
-                 dv.pitch, w, a1 - a0, dz1 - dz0, ((long long)sz0 * sv.ln[1][s] + (sa0 - sv.ls[1][s])) * sv.pitch,
-                 ((long long)dz0 * dv.ln[1][s] + (a0 - dv.ls[1][s])) * dv.pitch);
+                 dv.pitch, w, a1 - a0, dz1 - dz0, ((long long)sz0 * sv.ln[1][s] + (sa0 - sv.ls[1][s])) * sv.pitch + sx0,
+                 ((long long)dz0 * dv.ln[1][s] + (a0 - dv.ls[1][s])) * dv.pitch + dx0);
         }
       }
       // z-slab planes inside the box
@@ -461,8 +488,8 @@ void add_face_jobs(fdtd_ctx* c, std::vector<CopyJob>& jobs, Domain& dst, Domain&
           const int sa0 = a0 + dv.oz - sv.oz;
           if (sa0 >= sv.ls[2][s] && sa0 + (a1 - a0) <= sv.ls[2][s] + sv.ln[2][s])
             push(sv.psi[fam][2][s], dv.psi[fam][2][s], (long long)sv.ny * sv.pitch, sv.pitch, (long long)dv.ny * dv.pitch, dv.pitch, w,
-                 dy1 - dy0, a1 - a0, ((long long)(sa0 - sv.ls[2][s]) * sv.ny + sy0) * sv.pitch,
-                 ((long long)(a0 - dv.ls[2][s]) * dv.ny + dy0) * dv.pitch);
+                 dy1 - dy0, a1 - a0, ((long long)(sa0 - sv.ls[2][s]) * sv.ny + sy0) * sv.pitch + sx0,
+                 ((long long)(a0 - dv.ls[2][s]) * dv.ny + dy0) * dv.pitch + dx0);
         }
       }
     }
@@ -471,15 +498,17 @@ void add_face_jobs(fdtd_ctx* c, std::vector<CopyJob>& jobs, Domain& dst, Domain&
 
 int exchange_halos(fdtd_ctx* c) {
   if (c->doms.size() <= 1) return FDTD_OK;
-  const int ny = c->G.nd[1], nz = c->G.nd[2];
-  for (int axis = 1; axis <= 2; ++axis) {
+  const int nd[3] = {c->G.nd[0], c->G.nd[1], c->G.nd[2]};
+  for (int axis = 0; axis <= 2; ++axis) {
+    if (nd[axis] == 1) continue;
     std::vector<CopyJob> jobs;
     for (auto& d : c->doms) {
-      const int pos = axis == 1 ? d.cy : d.cz, cnt = axis == 1 ? ny : nz;
+      const int pos[3] = {d.cx, d.cy, d.cz};
       for (int side = 0; side < 2; ++side) {
-        const int npos = pos + (side == 0 ? -1 : 1);
-        if (npos < 0 || npos >= cnt) continue;
-        Domain& src = c->doms[axis == 1 ? (size_t)d.cz * ny + npos : (size_t)npos * ny + d.cy];
+        int np[3] = {pos[0], pos[1], pos[2]};
+        np[axis] += side == 0 ? -1 : 1;
+        if (np[axis] < 0 || np[axis] >= nd[axis]) continue;
+        Domain& src = c->doms[((size_t)np[2] * nd[1] + np[1]) * nd[0] + np[0]];
         add_face_jobs(c, jobs, d, src, axis, side);
       }
     }
@@ -537,27 +566,29 @@ bool all_positive_finite(const float* a, size_t n) {
 }
 
 // gather / scatter between a packed host total-grid array and the domains
-int copy_field(fdtd_ctx* c, float* const* dom_base, float* host, bool to_host, bool owned_only) {
+int copy_field(fdtd_ctx* c, float* const* dom_base_f, float* host_f, bool to_host, bool owned_only, size_t es = 4) {
   const int gnx = c->G.gn[0], gny = c->G.gn[1];
+  char* host = (char*)host_f;
   for (auto& d : c->doms) {
     const DomainView& v = d.v;
+    const int il = owned_only ? d.own_lo[0] : 0, ih = owned_only ? d.own_hi[0] : v.nx;
     const int jl = owned_only ? d.own_lo[1] : 0, jh = owned_only ? d.own_hi[1] : v.ny;
     const int kl = owned_only ? d.own_lo[2] : 0, kh = owned_only ? d.own_hi[2] : v.nz;
-    float* base = dom_base[&d - &c->doms[0]];
+    char* base = (char*)dom_base_f[&d - &c->doms[0]];
     if (jl == 0 && jh == v.ny && v.ny == gny && v.oy == 0) {
       // whole planes: rows of consecutive planes are consecutive on both sides -> one 2-D copy
-      float* dev = base + (long long)kl * v.plane;
-      float* h = host + (long long)(kl + v.oz) * gny * gnx;
+      char* dev = base + ((long long)kl * v.plane + il) * es;
+      char* h = host + ((long long)(kl + v.oz) * gny * gnx + (il + v.ox)) * es;
       const size_t rows = (size_t)(kh - kl) * v.ny;
-      if (to_host) CK(cudaMemcpy2DAsync(h, (size_t)gnx * 4, dev, (size_t)v.pitch * 4, (size_t)v.nx * 4, rows, cudaMemcpyDeviceToHost, c->stream));
-      else CK(cudaMemcpy2DAsync(dev, (size_t)v.pitch * 4, h, (size_t)gnx * 4, (size_t)v.nx * 4, rows, cudaMemcpyHostToDevice, c->stream));
+      if (to_host) CK(cudaMemcpy2DAsync(h, (size_t)gnx * es, dev, (size_t)v.pitch * es, (size_t)(ih - il) * es, rows, cudaMemcpyDeviceToHost, c->stream));
+      else CK(cudaMemcpy2DAsync(dev, (size_t)v.pitch * es, h, (size_t)gnx * es, (size_t)(ih - il) * es, rows, cudaMemcpyHostToDevice, c->stream));
       continue;
     }
     for (int k = kl; k < kh; ++k) {
-      float* dev = base + (long long)k * v.plane + (long long)jl * v.pitch;
-      float* h = host + ((long long)(k + v.oz) * gny + (jl + v.oy)) * gnx;
-      if (to_host) CK(cudaMemcpy2DAsync(h, (size_t)gnx * 4, dev, (size_t)v.pitch * 4, (size_t)v.nx * 4, jh - jl, cudaMemcpyDeviceToHost, c->stream));
-      else CK(cudaMemcpy2DAsync(dev, (size_t)v.pitch * 4, h, (size_t)gnx * 4, (size_t)v.nx * 4, jh - jl, cudaMemcpyHostToDevice, c->stream));
+      char* dev = base + ((long long)k * v.plane + (long long)jl * v.pitch + il) * es;
+      char* h = host + (((long long)(k + v.oz) * gny + (jl + v.oy)) * gnx + (il + v.ox)) * es;
+      if (to_host) CK(cudaMemcpy2DAsync(h, (size_t)gnx * es, dev, (size_t)v.pitch * es, (size_t)(ih - il) * es, jh - jl, cudaMemcpyDeviceToHost, c->stream));
+      else CK(cudaMemcpy2DAsync(dev, (size_t)v.pitch * es, h, (size_t)gnx * es, (size_t)(ih - il) * es, jh - jl, cudaMemcpyHostToDevice, c->stream));
     }
   }
   CK(cudaStreamSynchronize(c->stream));
@@ -565,6 +596,27 @@ int copy_field(fdtd_ctx* c, float* const* dom_base, float* host, bool to_host, b
 }
 
 }  // namespace
+
+template <class V>
+static int get_psi_impl(fdtd_ctx* c, Domain& d, const V& v, int fam, int axis, typename V::real* dst) {
+  typedef typename V::real T;
+  const int gnx = c->G.gn[0], gny = c->G.gn[1];
+  const size_t n = (size_t)v.nx * v.ny * v.nz;
+  T* tmp = nullptr;
+  CK(cudaMalloc(&tmp, n * sizeof(T)));                 // debug-only scratch, not field storage
+  expand_psi_kernel<<<148 * 8, 256, 0, c->stream>>>(v, fam, axis, tmp);
+  c->launches++;
+  for (int k = d.own_lo[2]; k < d.own_hi[2]; ++k) {
+    const T* dev = tmp + ((size_t)k * v.ny + d.own_lo[1]) * v.nx + d.own_lo[0];
+    T* h = dst + ((size_t)(k + v.oz) * gny + (d.own_lo[1] + v.oy)) * gnx + (d.own_lo[0] + v.ox);
+    cudaMemcpy2DAsync(h, (size_t)gnx * sizeof(T), dev, (size_t)v.nx * sizeof(T), (size_t)(d.own_hi[0] - d.own_lo[0]) * sizeof(T),
+                      d.own_hi[1] - d.own_lo[1], cudaMemcpyDeviceToHost, c->stream);
+  }
+  cudaError_t e = cudaStreamSynchronize(c->stream);
+  cudaFree(tmp);
+  CK(e);
+  return FDTD_OK;
+}
 
 // =========================================================================================== C ABI
 extern "C" {
@@ -603,7 +655,9 @@ fdtd_ctx* fdtd_create(const fdtd_params* P) {
   c->ws = (char*)P->workspace;
   c->stream = (cudaStream_t)P->stream;
   // the tiled kernels move whole float4s: they need Nx % 4 == 0; other grids take the reference kernels
-  c->use_ref = P->kernel == FDTD_KERNEL_REF || P->boundary == FDTD_PERIODIC || (G.gn[0] % 4) != 0;
+  c->fp64 = P->precision == FDTD_PRECISION_FP64;
+  c->es = c->fp64 ? 8 : 4;
+  c->use_ref = P->kernel == FDTD_KERNEL_REF || P->boundary == FDTD_PERIODIC || (G.gn[0] % 4) != 0 || c->fp64;
   c->fused = P->kernel == FDTD_KERNEL_FUSED;      // make_geometry has checked that the tiled path applies
   cudaError_t e;
   if ((e = cudaSetDevice(P->device)) != cudaSuccess) return fail(c, e, "cudaSetDevice");
@@ -638,7 +692,8 @@ fdtd_ctx* fdtd_create(const fdtd_params* P) {
 
   size_t di = 0;
   for (int cz = 0; cz < G.nd[2]; ++cz)
-    for (int cy = 0; cy < G.nd[1]; ++cy, ++di) {
+    for (int cy = 0; cy < G.nd[1]; ++cy)
+     for (int cx = 0; cx < G.nd[0]; ++cx, ++di) {
       const Layout::Dom& ld = L.doms[di];
       Domain d{};
       DomainView& v = d.v;
@@ -660,11 +715,26 @@ fdtd_ctx* fdtd_create(const fdtd_params* P) {
       for (int fam = 0; fam < 2; ++fam)
         for (int a = 0; a < 3; ++a)
           for (int k = 0; k < 3; ++k) v.tab[fam][a][k] = (const float*)(c->ws + L.tab[fam][a][k]);
-      d.cy = cy; d.cz = cz;
-      const int cc[3] = {0, cy, cz};
+      d.cx = cx; d.cy = cy; d.cz = cz;
+      const int cc[3] = {cx, cy, cz};
       for (int a = 0; a < 3; ++a) {
         d.own_lo[a] = cc[a] > 0 ? G.ghost : 0;
         d.own_hi[a] = d.own_lo[a] + G.gn[a] / G.nd[a];
+      }
+      if (c->fp64) {                                  // same geometry, double state
+        DomainViewT<double>& w = d.v64;
+        w.nx = v.nx; w.ny = v.ny; w.nz = v.nz; w.pitch = v.pitch; w.plane = v.plane; w.ox = v.ox; w.oy = v.oy; w.oz = v.oz;
+        w.periodic = v.periodic; w.kc = nullptr; w.kc0 = v.kc0; w.b0 = v.b0;
+        for (int a = 0; a < 3; ++a) {
+          w.gn[a] = v.gn[a]; w.bq[a] = nullptr;
+          for (int s = 0; s < 2; ++s) {
+            w.ls[a][s] = v.ls[a][s]; w.ln[a][s] = v.ln[a][s];
+            for (int fam = 0; fam < 2; ++fam) w.psi[fam][a][s] = (double*)(c->ws + ld.psi[fam][a][s]);
+          }
+          for (int fam = 0; fam < 2; ++fam)
+            for (int k = 0; k < 3; ++k) w.tab[fam][a][k] = v.tab[fam][a][k];
+        }
+        for (int f = 0; f < 4; ++f) w.f[f] = (double*)(c->ws + ld.f[f]);
       }
       d.src_offset = (long long*)(c->ws + ld.src_off);
       d.counters = (unsigned int*)(c->ws + ld.counters);
@@ -675,6 +745,10 @@ fdtd_ctx* fdtd_create(const fdtd_params* P) {
           int bad = make_tmap(enc, &tm.p_halo, f[0], v, HW, VH) || make_tmap(enc, &tm.vx_halo, f[1], v, HW, TY) ||
                     make_tmap(enc, &tm.vy_halo, f[2], v, TX, PH) || make_tmap(enc, &tm.p_box, f[0], v, BW, BH);
           for (int t = 0; t < 5 && !bad; ++t) bad = make_tmap(enc, &tm.tile[t], tile_base[t], v, TX, TY);
+          if (!bad && P->density == FDTD_DENSITY_ARRAY)
+            bad = make_tmap(enc, &tm.bq_halo[0], (float*)(c->ws + ld.bq[0]), v, HW, TY) ||
+                  make_tmap(enc, &tm.bq_halo[1], (float*)(c->ws + ld.bq[1]), v, TX, PH) ||
+                  make_tmap(enc, &tm.bq_tile, (float*)(c->ws + ld.bq[2]), v, TX, TY);
           return bad;
         };
         int bad = make_maps(d.tm, v.f);
@@ -701,9 +775,12 @@ fdtd_ctx* fdtd_create(const fdtd_params* P) {
         plan_launch(c, (const void*)update_p_tiled, P_SMEM_BYTES, &c->grid_p)) { delete c; return nullptr; }
     for (auto& d : c->doms) plan_items(d, std::min(c->grid_v, c->grid_p));
     if (c->fused) {
-      if ((e = cudaFuncSetAttribute(step_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, F_SMEM_BYTES)) != cudaSuccess)
+      if ((e = cudaFuncSetAttribute(step_fused<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, f_smem_bytes<false>())) != cudaSuccess ||
+          (e = cudaFuncSetAttribute(step_fused<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, f_smem_bytes<true>())) != cudaSuccess)
         return fail(c, e, "cudaFuncSetAttribute(step_fused)");
-      if (plan_launch(c, (const void*)step_fused, F_SMEM_BYTES, &c->grid_f, FNT)) { delete c; return nullptr; }
+      const bool hb = P->density == FDTD_DENSITY_ARRAY;
+      if (plan_launch(c, hb ? (const void*)step_fused<true> : (const void*)step_fused<false>, hb ? f_smem_bytes<true>() : f_smem_bytes<false>(),
+                      &c->grid_f, FNT)) { delete c; return nullptr; }
       for (size_t k = 0; k < c->doms.size(); ++k) {
         Domain& d = c->doms[k];
         std::vector<int4> table;
@@ -731,6 +808,14 @@ int64_t fdtd_launch_count(const fdtd_ctx* c) { return c ? c->launches : -1; }
 // dt/(rho_bar dx) at the half nodes of vx, vy, vz with rho_bar the mean of the two adjacent nodes (the last node of an
 // axis repeats itself; that half node is pinned anyway, R3).  Formed on the host in double from the fp32 inputs, rounded
 // once, then scattered to the domains (ghost cells included, so subdomains see the global neighbour).
+// the fp64 view shares the medium (fp32 coefficients) with the fp32 view
+static void sync_v64(fdtd_ctx* c) {
+  for (auto& d : c->doms) {
+    d.v64.kc = d.v.kc; d.v64.kc0 = d.v.kc0; d.v64.b0 = d.v.b0;
+    for (int a = 0; a < 3; ++a) d.v64.bq[a] = d.v.bq[a];
+  }
+}
+
 static int set_model_density_array(fdtd_ctx* c, const float* c_host, const float* rho_host) {
   if (c->P.density != FDTD_DENSITY_ARRAY) {
     set_err("a heterogeneous rho needs params.density = FDTD_DENSITY_ARRAY (the workspace must hold the three dt/(rho_bar dx) arrays)");
@@ -771,6 +856,7 @@ static int set_model_density_array(fdtd_ctx* c, const float* c_host, const float
     v.kc = bases[k];
     for (int a = 0; a < 3; ++a) v.bq[a] = (const float*)(c->ws + c->L.doms[k].bq[a]);
   }
+  sync_v64(c);
   return FDTD_OK;
 }
 
@@ -796,6 +882,7 @@ int fdtd_set_model(fdtd_ctx* c, const float* c_host, const float* rho_host) {
   const float b0 = (float)(c->P.dt / (rho * c->P.dx));
   if (!c_host) {
     for (auto& d : c->doms) { d.v.kc = nullptr; d.v.kc0 = (float)(rho * 1.0 * 1.0 * c->P.dt / c->P.dx); d.v.b0 = b0; }
+    sync_v64(c);
     return FDTD_OK;
   }
   // c goes up as fp32; K dt/dx = rho c^2 dt/dx (R6) is formed on the device in double and rounded once
@@ -811,6 +898,7 @@ int fdtd_set_model(fdtd_ctx* c, const float* c_host, const float* rho_host) {
   CK(cudaGetLastError());
   CK(cudaStreamSynchronize(c->stream));
   for (size_t k = 0; k < c->doms.size(); ++k) { c->doms[k].v.kc = bases[k]; c->doms[k].v.b0 = b0; }
+  sync_v64(c);
   return FDTD_OK;
 }
 
@@ -909,30 +997,49 @@ int fdtd_kernel_in_use(const fdtd_ctx* c) {
   return c->fused ? FDTD_KERNEL_FUSED : (c->use_ref ? FDTD_KERNEL_REF : FDTD_KERNEL_AUTO);
 }
 
-static int field_bases(fdtd_ctx* c, int which, std::vector<float*>& bases) {
+static int field_bases(fdtd_ctx* c, int which, std::vector<float*>& bases, bool want_f64) {
   if (which < 0 || which > 3) { set_err("bad field selector"); return FDTD_EINVAL; }
-  for (auto& d : c->doms) bases.push_back(d.v.f[which]);
+  if (want_f64 != c->fp64) {
+    set_err(c->fp64 ? "this context holds fp64 fields: use the _f64 entry points" : "this context holds fp32 fields: use the fp32 entry points");
+    return FDTD_EUNSUPPORTED;
+  }
+  for (auto& d : c->doms) bases.push_back(c->fp64 ? (float*)d.v64.f[which] : d.v.f[which]);
   return FDTD_OK;
 }
 
 int fdtd_get_field(fdtd_ctx* c, int32_t which, float* dst) {
   if (!c || !dst) return FDTD_EINVAL;
   std::vector<float*> b;
-  int r = field_bases(c, which, b);
+  int r = field_bases(c, which, b, false);
   return r ? r : copy_field(c, b.data(), dst, true, true);
 }
 
 int fdtd_set_field(fdtd_ctx* c, int32_t which, const float* src) {
   if (!c || !src) return FDTD_EINVAL;
   std::vector<float*> b;
-  int r = field_bases(c, which, b);
+  int r = field_bases(c, which, b, false);
   if (r) return r;
   c->substeps_done = 0;                       // ghosts are written consistently: restart the exchange cadence
   return copy_field(c, b.data(), const_cast<float*>(src), false, false);
 }
 
+int fdtd_get_field_f64(fdtd_ctx* c, int32_t which, double* dst) {
+  if (!c || !dst) return FDTD_EINVAL;
+  std::vector<float*> b;
+  int r = field_bases(c, which, b, true);
+  return r ? r : copy_field(c, b.data(), (float*)dst, true, true, 8);
+}
+
+int fdtd_set_field_f64(fdtd_ctx* c, int32_t which, const double* src) {
+  if (!c || !src) return FDTD_EINVAL;
+  std::vector<float*> b;
+  int r = field_bases(c, which, b, true);
+  return r ? r : copy_field(c, b.data(), (float*)const_cast<double*>(src), false, false, 8);
+}
+
 int fdtd_get_field_box(fdtd_ctx* c, int32_t which, const int32_t lo[3], const int32_t size[3], float* dst) {
   if (!c || !lo || !size || !dst || which < 0 || which > 3) return FDTD_EINVAL;
+  if (c->fp64) { set_err("fdtd_get_field_box reads fp32 fields: use fdtd_get_field_f64 on an fp64 context"); return FDTD_EUNSUPPORTED; }
   for (int a = 0; a < 3; ++a)
     if (lo[a] < 0 || size[a] <= 0 || lo[a] + size[a] > c->G.gn[a]) { set_err("box outside the grid"); return FDTD_EINVAL; }
   for (auto& d : c->doms) {
@@ -961,7 +1068,8 @@ int fdtd_get_field_box(fdtd_ctx* c, int32_t which, const int32_t lo[3], const in
 int fdtd_fill_hash(fdtd_ctx* c, int32_t which, uint64_t seed, double scale) {
   if (!c || which < 0 || which > 3) return FDTD_EINVAL;
   for (auto& d : c->doms) {
-    fill_hash_kernel<<<148 * 8, 256, 0, c->stream>>>(d.v, which, seed, (float)scale);
+    if (c->fp64) fill_hash_kernel<<<148 * 8, 256, 0, c->stream>>>(d.v64, which, seed, (float)scale);
+    else fill_hash_kernel<<<148 * 8, 256, 0, c->stream>>>(d.v, which, seed, (float)scale);
     c->launches++;
   }
   c->substeps_done = 0;
@@ -986,8 +1094,12 @@ int fdtd_field_absmax(fdtd_ctx* c, int32_t which, const int32_t lo[3], const int
       if (g1[a] <= g0[a]) empty = true;
     }
     if (empty) continue;
-    absmax_kernel<<<148 * 4, 256, 0, c->stream>>>(v, which, g0[0] - o[0], g0[1] - o[1], g0[2] - o[2], g1[0] - g0[0], g1[1] - g0[1],
-                                                  g1[2] - g0[2], acc);
+    if (c->fp64)
+      absmax_kernel<<<148 * 4, 256, 0, c->stream>>>(d.v64, which, g0[0] - o[0], g0[1] - o[1], g0[2] - o[2], g1[0] - g0[0], g1[1] - g0[1],
+                                                    g1[2] - g0[2], acc);
+    else
+      absmax_kernel<<<148 * 4, 256, 0, c->stream>>>(v, which, g0[0] - o[0], g0[1] - o[1], g0[2] - o[2], g1[0] - g0[0], g1[1] - g0[1],
+                                                    g1[2] - g0[2], acc);
     c->launches++;
   }
   CK(cudaGetLastError());
@@ -1000,23 +1112,20 @@ int fdtd_field_absmax(fdtd_ctx* c, int32_t which, const int32_t lo[3], const int
 
 int fdtd_get_psi(fdtd_ctx* c, int32_t which, float* dst) {
   if (!c || !dst || which < 0 || which > 5) return FDTD_EINVAL;
-  const int fam = which / 3, axis = which % 3;
-  const int gnx = c->G.gn[0], gny = c->G.gn[1];
+  if (c->fp64) { set_err("this context holds fp64 memory variables: use fdtd_get_psi_f64"); return FDTD_EUNSUPPORTED; }
   for (auto& d : c->doms) {
-    const DomainView& v = d.v;
-    const size_t n = (size_t)v.nx * v.ny * v.nz;
-    float* tmp = nullptr;
-    CK(cudaMalloc(&tmp, n * 4));                       // debug-only scratch, not field storage
-    expand_psi_kernel<<<148 * 8, 256, 0, c->stream>>>(v, fam, axis, tmp);
-    c->launches++;
-    for (int k = d.own_lo[2]; k < d.own_hi[2]; ++k) {
-      const float* dev = tmp + ((size_t)k * v.ny + d.own_lo[1]) * v.nx;
-      float* h = dst + ((size_t)(k + v.oz) * gny + (d.own_lo[1] + v.oy)) * gnx;
-      cudaMemcpyAsync(h, dev, (size_t)v.nx * (d.own_hi[1] - d.own_lo[1]) * 4, cudaMemcpyDeviceToHost, c->stream);
-    }
-    cudaError_t e = cudaStreamSynchronize(c->stream);
-    cudaFree(tmp);
-    CK(e);
+    int r = get_psi_impl(c, d, d.v, which / 3, which % 3, dst);
+    if (r) return r;
+  }
+  return FDTD_OK;
+}
+
+int fdtd_get_psi_f64(fdtd_ctx* c, int32_t which, double* dst) {
+  if (!c || !dst || which < 0 || which > 5) return FDTD_EINVAL;
+  if (!c->fp64) { set_err("this context holds fp32 memory variables: use fdtd_get_psi"); return FDTD_EUNSUPPORTED; }
+  for (auto& d : c->doms) {
+    int r = get_psi_impl(c, d, d.v64, which / 3, which % 3, dst);
+    if (r) return r;
   }
   return FDTD_OK;
 }

@@ -8,31 +8,36 @@
 // a ghost of 2r = 8 cells per full step, exactly the paper's count.  Inside one GPU that ghost is
 //   x, y : recomputed.  A 64x16 tile computes vx_new on 72x16 and vy_new on 64x23 points; the extra strips are done
 //          by four "halo" warps, the tile itself by eight "main" warps, and the values meet in a double-buffered
-//          shared-memory exchange (E) guarded by full/empty mbarriers;
-//   z    : streamed.  Each main thread keeps p_old[m-7..m] and vz_new[k-4..k+3] of its four x-points in registers.
+//          shared-memory exchange (E) guarded by one mbarrier per buffer;
+//   z    : streamed.  Each main thread keeps p_old[k..k+7] and vz_new[k-4..k+3] of its four x-points in registers.
 // Because neighbouring tiles re-read old values that the owner is about to overwrite, the step is out of place:
 // state "in" -> state "out" (fields and psi), swapped by the host after every launch.
 //
 // Stage of ring iteration m (k = m-7 is the output plane, kz = m-4 the vz plane), all by TMA, OOB = 0 = wall (R4):
 //   [ p box (TX+16)x(TY+14) of plane k | p tile of plane m | vz tile of plane kz | vx x-halo tile of plane k |
-//     vy y-halo tile of plane k | Kc tile of plane k ]
+//     vy y-halo tile of plane k | Kc tile of plane k | HB: bx x-halo tile, by y-halo tile of plane k, bz tile of plane kz ]
+// (HB = heterogeneous density: dt/(rho_bar dx) per half node, FDTD_DENSITY_ARRAY, reading R6.)
+//
+// Roles (one CTA of 512 threads per SM, registers redistributed with setmaxnreg):
+//   warps 0-7   main     one float4 of the tile per thread; planes that cannot touch a z slab run an instantiation of the
+//                        plane body without any z-slab code, items that touch no x / y slab one without x / y slab code
+//   warps 8-11  halo     the recomputed ghost strips (never stored to global memory)
+//   warps 12-15 producer lane 0 of warp 12 issues every TMA load and does nothing else (a lane that has just issued
+//                        tensor copies sees its own shared-memory loads stall for about a thousand cycles)
 #pragma once
 #include "fdtd_kernels.cuh"
 
 namespace fdtd {
 
-constexpr int FW_MAIN = NT / 32;                 // 8 main warps: one float4 of the 64x16 tile per thread
-constexpr int FW_HALO = 4;                       // one warpgroup: vy_new on rows y0-4..y0-1 and y0+TY..y0+TY+2 (7 x 16 float4
-                                                 // units, two rows per warp) and, by its last warp, vx_new on the two 4-wide
-                                                 // strips left/right of the tile (2 x 16 units)
-constexpr int FW_PROD = 4;                       // one warpgroup whose first lane issues every TMA load and does nothing else: a
-                                                 // lane that has just issued tensor copies sees its own shared-memory loads stall
-                                                 // for about a thousand cycles, which made a producing halo warp the slowest warp
-                                                 // of the CTA (traced with clock64, see profiles/r01b_ncu_config3.md)
+constexpr int FW_MAIN = NT / 32;                 // 8 main warps
+constexpr int FW_HALO = 4;                       // vy_new on rows y0-4..y0-1 and y0+TY..y0+TY+2 (7 x 16 float4 units, two rows
+                                                 // per warp); the last warp also does vx_new on the two 4-wide strips
+constexpr int FW_PROD = 4;                       // producer warpgroup (one working lane)
 constexpr int FNW = FW_MAIN + FW_HALO;           // 12 consumer warps
 constexpr int FNT = (FNW + FW_PROD) * 32;        // 512 threads = 4 warps per SM sub-partition
-constexpr int F_REGS_MAIN = 200, F_REGS_HALO = 80, F_REGS_PROD = 32;   // setmaxnreg split of 4 x 128 registers per sub-partition lane
+constexpr int F_REGS_MAIN = 200, F_REGS_HALO = 80, F_REGS_PROD = 32;   // 2 x 200 + 80 + 32 = 512 registers per sub-partition lane
 constexpr int FNS = 4;                           // TMA ring stages
+constexpr int F_LEAD = 14;                       // ring iterations of an item before its first output plane
 constexpr int BW = TX + 16;                      // p box: columns x0-8 .. x0+TX+7
 constexpr int BH = TY + 14;                      // p box: rows    y0-7 .. y0+TY+6
 constexpr int EVY_ROWS = TY + 8;                 // vy_new exchange rows y0-4 .. y0+TY+3 (the last one is never read)
@@ -44,12 +49,16 @@ constexpr int F_OFF_VZ = F_OFF_PT + TILE_FLOATS;
 constexpr int F_OFF_VX = F_OFF_VZ + TILE_FLOATS;
 constexpr int F_OFF_VY = F_OFF_VX + F_VX_FLOATS;
 constexpr int F_OFF_KC = F_OFF_VY + F_VY_FLOATS;
-constexpr int F_STAGE_FLOATS = F_OFF_KC + TILE_FLOATS;
+constexpr int F_OFF_BX = F_OFF_KC + TILE_FLOATS; // HB only
+constexpr int F_OFF_BY = F_OFF_BX + F_VX_FLOATS;
+constexpr int F_OFF_BZ = F_OFF_BY + F_VY_FLOATS;
+template <bool HB> __host__ __device__ constexpr int f_stage_floats() { return HB ? F_OFF_BZ + TILE_FLOATS : F_OFF_BX; }
 constexpr int E_OFF_VY = F_VX_FLOATS;            // exchange buffer: [vx_new 16 x 72 | vy_new 24 x 64]
 constexpr int E_FLOATS = F_VX_FLOATS + TX * EVY_ROWS;
-constexpr int F_SMEM_BYTES = (FNS * F_STAGE_FLOATS + 2 * E_FLOATS) * 4;
+template <bool HB> __host__ __device__ constexpr int f_smem_bytes() { return (FNS * f_stage_floats<HB>() + 2 * E_FLOATS) * 4; }
 static_assert((F_PB_FLOATS * 4) % 128 == 0 && (F_VX_FLOATS * 4) % 128 == 0 && (F_VY_FLOATS * 4) % 128 == 0 && (E_FLOATS * 4) % 128 == 0,
               "TMA destinations must stay 128-B aligned");
+static_assert(f_smem_bytes<true>() <= 227 * 1024 - 4096, "stage ring + exchange buffers + static shared memory must fit one SM");
 
 // The "out" state of a fused step (same layout as the DomainView's own arrays, which are the "in" state).
 struct OutSet {
@@ -57,9 +66,7 @@ struct OutSet {
   float* psi[2][3][2];
 };
 
-// CPML tables of the item's columns x0-4 .. x0+TX+3 and rows y0-4 .. y0+TY+3 in shared memory ([family][a, b, 1/kappa]):
-// the per-plane table reads of the slab items were global loads issued right before their use (long-scoreboard stalls
-// in the source view); from here they are LDS next to the other shared-memory reads of the plane.
+// CPML tables of the item's columns x0-4 .. x0+TX+3 and rows y0-4 .. y0+TY+3 in shared memory ([family][a, b, 1/kappa]).
 constexpr int TCX = HW, TCY = TY + 8;
 struct TabCache {
   float x[2][3][TCX];
@@ -92,251 +99,307 @@ __device__ __forceinline__ void warp_arrive(uint64_t* bar) {
   if ((threadIdx.x & 31) == 0) mbar_arrive(bar);
 }
 
+template <bool HB>
 __device__ __forceinline__ void fused_issue(const TMaps& tm, float* smem, uint64_t* full, unsigned slot, int m, int x0, int y0, int z0,
                                             bool has_kc) {
   const int k = m - 7;
   const bool vz = m >= z0, out = k >= z0;
   uint64_t* bar = &full[slot];
-  float* st = smem + slot * F_STAGE_FLOATS;
-  mbar_expect_tx(bar, TILE_BYTES + (vz ? TILE_BYTES : 0) +
-                          (out ? (F_PB_FLOATS + F_VX_FLOATS + F_VY_FLOATS) * 4 + (has_kc ? TILE_BYTES : 0) : 0));
+  float* st = smem + slot * f_stage_floats<HB>();
+  mbar_expect_tx(bar, TILE_BYTES + (vz ? (HB ? 2 : 1) * TILE_BYTES : 0) +
+                          (out ? (F_PB_FLOATS + (HB ? 2 : 1) * (F_VX_FLOATS + F_VY_FLOATS)) * 4 + (has_kc ? TILE_BYTES : 0) : 0));
   tma_load_3d(st + F_OFF_PT, &tm.tile[0], bar, x0, y0, m);
-  if (vz) tma_load_3d(st + F_OFF_VZ, &tm.tile[3], bar, x0, y0, m - 4);
+  if (vz) {
+    tma_load_3d(st + F_OFF_VZ, &tm.tile[3], bar, x0, y0, m - 4);
+    if (HB) tma_load_3d(st + F_OFF_BZ, &tm.bq_tile, bar, x0, y0, m - 4);
+  }
   if (out) {
     tma_load_3d(st, &tm.p_box, bar, x0 - 8, y0 - 7, k);
     tma_load_3d(st + F_OFF_VX, &tm.vx_halo, bar, x0 - 4, y0, k);
     tma_load_3d(st + F_OFF_VY, &tm.vy_halo, bar, x0, y0 - 4, k);
     if (has_kc) tma_load_3d(st + F_OFF_KC, &tm.tile[4], bar, x0, y0, k);
+    if (HB) {
+      tma_load_3d(st + F_OFF_BX, &tm.bq_halo[0], bar, x0 - 4, y0, k);
+      tma_load_3d(st + F_OFF_BY, &tm.bq_halo[1], bar, x0, y0 - 4, k);
+    }
   }
 }
 
 // ---- main warps: the tile's own points ------------------------------------------------------------------
-// Per-thread state of a main thread over one item.  The two z queues are arrays that are only ever indexed with
-// compile-time constants (the steady loop is unrolled 8x so that the rotation is a renaming, not a move).
-struct MainCtx {
-  V4 pq[8];                 // p_old ring:  canonical order pq[n] = p_old[m-7+n]
-  V4 wq[8];                 // vz_new ring: canonical order wq[n] = vz_new[kz-7+n]
-  float* gvx; float* gvy; float* gvz; float* gp;      // output pointers of the current planes (k, k, kz, k)
-  long long pox, poy;       // psi offsets of plane k in the x / y slab arrays (same in psi_v / psi_p, in / out)
-  V4 nvx, nvy, npx, npy;    // psi_v / psi_p of plane k, loaded one iteration ahead (items that touch an x / y slab)
+// Everything a main thread keeps over one item.  The two z queues are arrays that are only ever indexed with
+// compile-time constants, so they live in registers.
+template <bool XS, bool YS>
+struct MainState {
+  V4 pq[8];                 // p_old ring:  logical entry n (after the push of plane k) = p_old[k+n]
+  V4 wq[8];                 // vz_new ring: logical entry n (after the push of plane k) = vz_new[k-4+n]
+  long long goff;           // element offset of this thread's float4 in plane k of a field
+  long long pox, poy;       // element offsets of plane k in the x / y slab psi arrays
+  V4 nvx, npx, nvy, npy;    // psi_v / psi_p of plane k, loaded one iteration ahead (XS / YS items)
   unsigned it, eit;
   bool pre;                 // the next stage's "full" phase was already seen complete by an early probe
 };
 
-struct MainConst {
-  int i, j, tx, ty, boff, toff, exo, eyo, sx, sy, gi, gj, z0, z1, zl, zh;
+// per-item constants of a main thread
+struct MainK {
+  int boff, toff, exo;      // own float4 (float offsets) in the p box, in a plain tile, in an x-halo tile (vx, E.vx, bx)
+  int tx, ty;
+  int z1, zv_end;           // last output plane + 1; vz planes >= zv_end belong to the next z chunk
+  int zl, zh;               // z slabs: local planes [0, zl) and [zh, nz)
+  int kz_pin;               // vz planes >= kz_pin take a zero update coefficient (pinned last half node R3, and planes above the grid)
+  float B, Bx3, By, kc0;
+  bool active, in_x, in_y, has_kc;
+  int sxs, sys;             // slab side (0 / 1) of this thread's columns / row when in_x / in_y
   long long stride_px, stride_py, zrow;
-  float Bxy, Bx3, By;
-  bool active, has_kc;
-  const TabCache* T;
+  const float* psi_in[2][2];   // [family][0 = x slab, 1 = y slab] of the slab side this thread lies in (in state)
+  float* psi_out[2][2];
 };
 
-__device__ __forceinline__ void shift_push(V4 (&q)[8], const V4& v) {
-#pragma unroll
-  for (int n = 0; n < 7; ++n) q[n] = q[n + 1];
-  q[7] = v;
-}
-
-// vz_new[kz] from the p ring (logical order a[0..7] = p_old[kz-3 .. kz+4]), CPML in the z slabs, store if owned.
-__device__ __forceinline__ V4 fused_vz(const DomainView& D, const OutSet& O, const MainConst& K, MainCtx& C, const V4& a0, const V4& a1,
-                                       const V4& a2, const V4& a3, const V4& a4, const V4& a5, const V4& a6, const V4& a7, V4 vz4, int kz) {
+// vz_new[kz] from the p ring (a0..a7 = p_old[kz-3 .. kz+4]); CPML in the z slabs; stored if this item owns the plane.
+template <bool HB, bool ZS>
+__device__ __forceinline__ V4 fused_vz(const DomainView& D, const OutSet& O, const MainK& K, const V4& a0, const V4& a1, const V4& a2,
+                                       const V4& a3, const V4& a4, const V4& a5, const V4& a6, const V4& a7, V4 vz4, const V4& bz4, int kz,
+                                       long long goff_kz, bool own) {
   V4 dzv = diff_8(a4, a3, a5, a2, a6, a1, a7, a0);
-  const int gk = kz + D.oz;
-  const bool inz = kz >= 0 && kz < D.nz;
-  if (__builtin_expect(inz && (kz < K.zl || kz >= K.zh), 0)) {   // block-uniform: this plane lies in a z slab (few planes do)
+  if (ZS && (unsigned)(kz - K.zl) >= (unsigned)(K.zh - K.zl) && (unsigned)kz < (unsigned)D.nz) {   // block-uniform: z slab
     const int sz = kz < K.zl ? 0 : 1;
+    const int gk = kz + D.oz;
     const long long poz = (long long)(kz - D.ls[2][sz]) * D.plane + K.zrow;
     const float ta = __ldg(D.tab[0][2][0] + gk), tb = __ldg(D.tab[0][2][1] + gk), tk = __ldg(D.tab[0][2][2] + gk);
     V4 psz = K.active ? ldg4(D.psi[0][2][sz] + poz) : zero4();
     cpml4s(dzv, psz, ta, tb, tk);
-    if (K.active && kz >= K.z0 && kz < K.z1) st4(O.psi[0][2][sz] + poz, psz);     // lead-in / tail planes belong to another item
+    if (own) st4(O.psi[0][2][sz] + poz, psz);
   }
-  const float Bz = (!inz || gk == D.gn[2] - 1) ? 0.f : K.Bxy;
-  vz4 = upd4(vz4, Bz, Bz, Bz, dzv);
-  if (K.active && kz >= K.z0 && kz < K.z1) st4(C.gvz, vz4);
-  C.gvz += D.plane;
+  if (HB) {
+    const bool pin = (unsigned)kz >= (unsigned)K.kz_pin;             // also planes below the grid (kz < 0): v outside is 0 (R4)
+#pragma unroll
+    for (int e = 0; e < 4; ++e) vz4.v[e] = upd(vz4.v[e], pin ? 0.f : bz4.v[e], dzv.v[e]);
+  } else {
+    const float Bz = (unsigned)kz >= (unsigned)K.kz_pin ? 0.f : K.B;
+    vz4 = upd4(vz4, Bz, Bz, Bz, dzv);
+  }
+  if (own) st4(O.f[3] + goff_kz, vz4);
   return vz4;
 }
 
-// One steady-state iteration: output plane k (m = k+7, kz = k+3).  R = rotation of the two rings on entry.
-template <int R, bool XY>
-__device__ __forceinline__ void fused_steady(const DomainView& D, const OutSet& O, const float* smem, float* ebuf, const FusedBars& Q,
-                                             const MainConst& K, MainCtx& C, int k) {
+// One steady-state iteration: output plane k (m = k+7, kz = k+3).  R = position of the oldest ring entry on entry.
+// ZS = this plane or its vz plane may lie in a z slab (the lean instantiation carries no z-slab code at all).
+template <int R, bool ZS, bool XS, bool YS, bool HB>
+__device__ __forceinline__ void fused_plane(const DomainView& D, const OutSet& O, const float* smem, float* ebuf, const FusedBars& Q,
+                                            const TabCache& T, const MainK& K, MainState<XS, YS>& C, int k) {
 #define PQ(n) C.pq[(R + 1 + (n)) & 7]
 #define WQ(n) C.wq[(R + 1 + (n)) & 7]
-  static_assert(R == 7, "canonical ring order: the rings are shifted, not renamed (an 8x unrolled body thrashes the 32 KB I-cache)");
   const unsigned slot = C.it % FNS;
-  const float* st = smem + slot * F_STAGE_FLOATS;
+  const float* st = smem + slot * f_stage_floats<HB>();
   // psi of plane k arrived during the previous iteration; start the loads of plane k+1 now
   V4 psx, psy, ppx, ppy;
-  if (XY) {
-    psx = C.nvx; psy = C.nvy; ppx = C.npx; ppy = C.npy;
-    if (k + 1 < K.z1) {
-      if (K.sx >= 0) { C.nvx = ldg4(D.psi[0][0][K.sx] + C.pox + K.stride_px); C.npx = ldg4(D.psi[1][0][K.sx] + C.pox + K.stride_px); }
-      if (K.sy >= 0) { C.nvy = ldg4(D.psi[0][1][K.sy] + C.poy + K.stride_py); C.npy = ldg4(D.psi[1][1][K.sy] + C.poy + K.stride_py); }
-    }
+  if (XS) {
+    psx = C.nvx; ppx = C.npx;
+    if (K.in_x && k + 1 < K.z1) { C.nvx = ldg4(K.psi_in[0][0] + C.pox + K.stride_px); C.npx = ldg4(K.psi_in[1][0] + C.pox + K.stride_px); }
+  }
+  if (YS) {
+    psy = C.nvy; ppy = C.npy;
+    if (K.in_y && k + 1 < K.z1) { C.nvy = ldg4(K.psi_in[0][1] + C.poy + K.stride_py); C.npy = ldg4(K.psi_in[1][1] + C.poy + K.stride_py); }
   }
   if (!C.pre) mbar_wait(&Q.full[slot], (C.it / FNS) & 1);
-  shift_push(C.pq, ld4(st + F_OFF_PT + K.toff));                // newest p_old plane: PQ(7)
+  C.pq[R] = ld4(st + F_OFF_PT + K.toff);                         // newest p_old plane k+7 replaces p_old[k-1]
   const float* row = st + K.boff;
   const V4 c = ld4(row);
   V4 dxv = diff_x<true>(ld4(row - 4), c, ld4(row + 4));
   V4 dyv = diff_8(ld4(row + BW), c, ld4(row + 2 * BW), ld4(row - BW), ld4(row + 3 * BW), ld4(row - 2 * BW), ld4(row + 4 * BW),
                   ld4(row - 3 * BW));
   V4 vx4 = ld4(st + F_OFF_VX + K.exo);
-  V4 vy4 = ld4(st + F_OFF_VY + (K.ty + 4) * TX + 4 * K.tx);
+  V4 vy4 = ld4(st + F_OFF_VY + 4 * TX + K.toff);
   V4 vz4 = ld4(st + F_OFF_VZ + K.toff);
-  const V4 kc4 = K.has_kc ? ld4(st + F_OFF_KC + K.toff) : splat4(D.kc0);
+  const V4 kc4 = K.has_kc ? ld4(st + F_OFF_KC + K.toff) : splat4(K.kc0);
+  V4 bx4, by4, bz4;
+  if (HB) { bx4 = ld4(st + F_OFF_BX + K.exo); by4 = ld4(st + F_OFF_BY + 4 * TX + K.toff); bz4 = ld4(st + F_OFF_BZ + K.toff); }
   warp_arrive(&Q.empty[slot]);
 
   // ---- velocity sub-update at plane k
-  if (XY) {
-    if (K.sx >= 0) {
-      cpml4(dxv, psx, ld4(K.T->x[0][0] + 4 + 4 * K.tx), ld4(K.T->x[0][1] + 4 + 4 * K.tx), ld4(K.T->x[0][2] + 4 + 4 * K.tx));
-      st4(O.psi[0][0][K.sx] + C.pox, psx);
-    }
-    if (K.sy >= 0) {
-      cpml4s(dyv, psy, K.T->y[0][0][4 + K.ty], K.T->y[0][1][4 + K.ty], K.T->y[0][2][4 + K.ty]);
-      st4(O.psi[0][1][K.sy] + C.poy, psy);
+  if (XS) {
+    if (K.in_x) {
+      cpml4(dxv, psx, ld4(T.x[0][0] + 4 + 4 * K.tx), ld4(T.x[0][1] + 4 + 4 * K.tx), ld4(T.x[0][2] + 4 + 4 * K.tx));
+      st4(K.psi_out[0][0] + C.pox, psx);
     }
   }
-  vx4 = upd4(vx4, K.Bxy, K.Bxy, K.Bx3, dxv);
-  vy4 = upd4(vy4, K.By, K.By, K.By, dyv);
-  if (K.active) { st4(C.gvx, vx4); st4(C.gvy, vy4); }
+  if (YS) {
+    if (K.in_y) {
+      cpml4s(dyv, psy, T.y[0][0][4 + K.ty], T.y[0][1][4 + K.ty], T.y[0][2][4 + K.ty]);
+      st4(K.psi_out[0][1] + C.poy, psy);
+    }
+  }
+  if (HB) {
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      vx4.v[e] = upd(vx4.v[e], (e == 3 && K.Bx3 == 0.f) ? 0.f : bx4.v[e], dxv.v[e]);
+      vy4.v[e] = upd(vy4.v[e], K.By == 0.f ? 0.f : by4.v[e], dyv.v[e]);
+    }
+  } else {
+    vx4 = upd4(vx4, K.B, K.B, K.Bx3, dxv);
+    vy4 = upd4(vy4, K.By, K.By, K.By, dyv);
+  }
+  if (K.active) { st4(O.f[1] + C.goff, vx4); st4(O.f[2] + C.goff, vy4); }
   const unsigned eb = C.eit & 1;
   float* E = ebuf + eb * E_FLOATS;
   // every main warp has passed the efull wait of the previous plane, so nobody still reads this buffer (see step_fused)
   st4(E + K.exo, vx4);
-  st4(E + K.eyo, vy4);
+  st4(E + E_OFF_VY + 4 * TX + K.toff, vy4);
   warp_arrive(&Q.efull[eb]);
 
   // ---- vz_new at kz+1/2 from p_old[kz-3 .. kz+4], then D-_z of the new vz ring
-  vz4 = fused_vz(D, O, K, C, PQ(0), PQ(1), PQ(2), PQ(3), PQ(4), PQ(5), PQ(6), PQ(7), vz4, k + 3);
-  shift_push(C.wq, vz4);                                         // WQ(7) = vz_new[k+3]
+  C.wq[R] = fused_vz<HB, ZS>(D, O, K, PQ(0), PQ(1), PQ(2), PQ(3), PQ(4), PQ(5), PQ(6), PQ(7), vz4, bz4, k + 3, C.goff + 3 * D.plane,
+                         K.active && k < K.zv_end);
   V4 dzp = diff_8(WQ(4), WQ(3), WQ(5), WQ(2), WQ(6), WQ(1), WQ(7), WQ(0));
   V4 ppz;
-  const bool pz = k < K.zl || k >= K.zh;                         // block-uniform: plane k lies in a z slab
+  const bool pz = ZS && (unsigned)(k - K.zl) >= (unsigned)(K.zh - K.zl);    // block-uniform: plane k lies in a z slab
   const int szp = k < K.zl ? 0 : 1;
-  const long long pozp = (long long)(k - D.ls[2][szp]) * D.plane + K.zrow;
-  if (__builtin_expect(pz, 0)) ppz = K.active ? ldg4(D.psi[1][2][szp] + pozp) : zero4();
+  long long pozp = 0;
+  if (pz) {
+    pozp = (long long)(k - D.ls[2][szp]) * D.plane + K.zrow;
+    ppz = K.active ? ldg4(D.psi[1][2][szp] + pozp) : zero4();
+  }
 
   // ---- pressure sub-update at plane k
   C.pre = mbar_test(&Q.full[(C.it + 1) % FNS], ((C.it + 1) / FNS) & 1);      // probe the next stage now, use the answer next iteration
   mbar_wait(&Q.efull[eb], (C.eit >> 1) & 1);
   const float* xr = E + K.exo;
   V4 dxp = diff_x<false>(ld4(xr - 4), vx4, ld4(xr + 4));
-  const float* col = E + E_OFF_VY + K.ty * TX + 4 * K.tx;         // row ty of E.vy <-> y = j-4
+  const float* col = E + E_OFF_VY + K.toff;                       // row ty of E.vy <-> y = j-4
   V4 dyp = diff_8(vy4, ld4(col + 3 * TX), ld4(col + 5 * TX), ld4(col + 2 * TX), ld4(col + 6 * TX), ld4(col + TX), ld4(col + 7 * TX),
                   ld4(col));
-  if (XY) {
-    if (K.sx >= 0) {
-      cpml4(dxp, ppx, ld4(K.T->x[1][0] + 4 + 4 * K.tx), ld4(K.T->x[1][1] + 4 + 4 * K.tx), ld4(K.T->x[1][2] + 4 + 4 * K.tx));
-      st4(O.psi[1][0][K.sx] + C.pox, ppx);
+  if (XS) {
+    if (K.in_x) {
+      cpml4(dxp, ppx, ld4(T.x[1][0] + 4 + 4 * K.tx), ld4(T.x[1][1] + 4 + 4 * K.tx), ld4(T.x[1][2] + 4 + 4 * K.tx));
+      st4(K.psi_out[1][0] + C.pox, ppx);
       C.pox += K.stride_px;
     }
-    if (K.sy >= 0) {
-      cpml4s(dyp, ppy, K.T->y[1][0][4 + K.ty], K.T->y[1][1][4 + K.ty], K.T->y[1][2][4 + K.ty]);
-      st4(O.psi[1][1][K.sy] + C.poy, ppy);
+  }
+  if (YS) {
+    if (K.in_y) {
+      cpml4s(dyp, ppy, T.y[1][0][4 + K.ty], T.y[1][1][4 + K.ty], T.y[1][2][4 + K.ty]);
+      st4(K.psi_out[1][1] + C.poy, ppy);
       C.poy += K.stride_py;
     }
   }
-  if (__builtin_expect(pz, 0)) {
+  if (pz) {
     const int gk = k + D.oz;
     cpml4s(dzp, ppz, __ldg(D.tab[1][2][0] + gk), __ldg(D.tab[1][2][1] + gk), __ldg(D.tab[1][2][2] + gk));
     if (K.active) st4(O.psi[1][2][szp] + pozp, ppz);
   }
   const float2 s0 = __fadd2_rn(__fadd2_rn(lo2(dxp), lo2(dyp)), lo2(dzp)), s1 = __fadd2_rn(__fadd2_rn(hi2(dxp), hi2(dyp)), hi2(dzp));
-  const V4 p4 = join2(__ffma2_rn(pk(-kc4.v[0], -kc4.v[1]), s0, lo2(PQ(0))), __ffma2_rn(pk(-kc4.v[2], -kc4.v[3]), s1, hi2(PQ(0))));
-  if (K.active) st4(C.gp, p4);
-  C.gvx += D.plane; C.gvy += D.plane; C.gp += D.plane;
+  const V4 p4 = join2(mad2(pk(-kc4.v[0], -kc4.v[1]), s0, lo2(PQ(0))), mad2(pk(-kc4.v[2], -kc4.v[3]), s1, hi2(PQ(0))));
+  if (K.active) st4(O.f[0] + C.goff, p4);
+  C.goff += D.plane;
   ++C.it; ++C.eit;
 #undef PQ
 #undef WQ
 }
 
-template <bool XY>
+// Planes [k, kend) of an item.  Both rings stay in canonical order (oldest entry at index 0): they are shifted by one entry
+// per plane (56 register moves).  Renaming instead of moving needs the body unrolled 8x (or 4x / 2x with a rotation per
+// group), and every unrolled form measured slower than this one (8x: 2.06 instead of 1.44 ms at 552^3, 4x: 1.51, 2x: 1.50):
+// the body must stay resident in the instruction cache, and the kernel is not bound by issue slots.
+template <bool ZS, bool XS, bool YS, bool HB>
+__device__ __forceinline__ void fused_run(const DomainView& D, const OutSet& O, const float* smem, float* ebuf, const FusedBars& Q,
+                                          const TabCache& T, const MainK& K, MainState<XS, YS>& C, int k, int kend) {
+  for (; k < kend; ++k) {
+#pragma unroll
+    for (int n = 0; n < 7; ++n) { C.pq[n] = C.pq[n + 1]; C.wq[n] = C.wq[n + 1]; }
+    fused_plane<7, ZS, XS, YS, HB>(D, O, smem, ebuf, Q, T, K, C, k);       // writes the newest entries at index 7
+  }
+}
+
+template <bool XS, bool YS, bool HB>
 __device__ __forceinline__ void fused_main_item(const DomainView& D, const OutSet& O, const float* smem, float* ebuf, const FusedBars& Q,
-                                                const MainConst& K, MainCtx& C) {
-  const int z0 = K.z0, z1 = K.z1;
+                                             const TabCache& T, unsigned& it_io, unsigned& eit_io, int x0, int y0, int z0, int z1) {
+  const int tid = threadIdx.x;
+  MainK K;
+  K.tx = tid & 15; K.ty = tid >> 4;
+  const int i = x0 + 4 * K.tx, j = y0 + K.ty;
+  K.z1 = z1; K.zv_end = z1 - 3;
+  K.has_kc = D.kc != nullptr;
+  K.kc0 = D.kc0;
+  K.active = (i < D.nx) && (j < D.ny);
+  K.B = K.active ? D.b0 : 0.f;
+  K.Bx3 = (i + 3 + D.ox) == D.gn[0] - 1 ? 0.f : (HB ? 1.f : K.B);     // pinned last half node (R3); HB: only the zero matters
+  K.By = (j + D.oy) == D.gn[1] - 1 ? 0.f : (HB ? 1.f : K.B);
+  K.kz_pin = min(D.gn[2] - 1 - D.oz, D.nz);
+  K.zrow = (long long)j * D.pitch + i;
+  K.boff = (K.ty + 7) * BW + 4 * K.tx + 8;
+  K.toff = K.ty * TX + 4 * K.tx;
+  K.exo = K.ty * HW + 4 * K.tx + 4;
+  K.zl = D.ln[2][0];                                                // low z slab = local planes [0, zl)
+  K.zh = D.ln[2][1] > 0 ? D.ls[2][1] : 0x3fffffff;                  // high z slab = local planes [zh, nz)
+  const int sx = (XS && K.active) ? slab_side(D, 0, i) : -1;
+  const int sy = (YS && K.active) ? slab_side(D, 1, j) : -1;
+  K.in_x = sx >= 0; K.in_y = sy >= 0;
+  K.sxs = max(sx, 0); K.sys = max(sy, 0);
+  K.stride_px = K.in_x ? (long long)D.ny * D.ln[0][K.sxs] : 0;
+  K.stride_py = K.in_y ? (long long)D.ln[1][K.sys] * D.pitch : 0;
+#pragma unroll
+  for (int fam = 0; fam < 2; ++fam) {
+    K.psi_in[fam][0] = D.psi[fam][0][K.sxs]; K.psi_out[fam][0] = O.psi[fam][0][K.sxs];
+    K.psi_in[fam][1] = D.psi[fam][1][K.sys]; K.psi_out[fam][1] = O.psi[fam][1][K.sys];
+  }
+  MainState<XS, YS> C;
+  C.it = it_io; C.eit = eit_io; C.pre = false;
+  C.pox = K.in_x ? psi_index(D, 0, K.sxs, i, j, z0) : 0;
+  C.poy = K.in_y ? psi_index(D, 1, K.sys, i, j, z0) : 0;
+  C.goff = K.zrow + (long long)z0 * D.plane;
 #pragma unroll
   for (int n = 0; n < 8; ++n) { C.pq[n] = zero4(); C.wq[n] = zero4(); }
-  // lead-in 1: planes z0-7 .. z0-1 of p_old only fill the ring
+  constexpr int SF = f_stage_floats<HB>();
+  // lead-in 1: planes z0-7 .. z0-1 of p_old only fill the ring (canonical order: shifted, not renamed)
   for (int m = z0 - 7; m < z0; ++m, ++C.it) {
     const unsigned slot = C.it % FNS;
     if (!C.pre) mbar_wait(&Q.full[slot], (C.it / FNS) & 1);
-    const V4 v = ld4(smem + slot * F_STAGE_FLOATS + F_OFF_PT + K.toff);
+    const V4 v = ld4(smem + slot * SF + F_OFF_PT + K.toff);
     warp_arrive(&Q.empty[slot]);
     C.pre = mbar_test(&Q.full[(C.it + 1) % FNS], ((C.it + 1) / FNS) & 1);
-    shift_push(C.pq, v);
+#pragma unroll
+    for (int n = 0; n < 7; ++n) C.pq[n] = C.pq[n + 1];
+    C.pq[7] = v;
   }
-  // lead-in 2: planes z0 .. z0+6 also produce vz_new[z0-4 .. z0+2]
+  // lead-in 2: planes z0 .. z0+6 also produce vz_new[z0-4 .. z0+2] (the first four belong to the z chunk below)
   for (int m = z0; m < z0 + 7; ++m, ++C.it) {
     const unsigned slot = C.it % FNS;
-    const float* st = smem + slot * F_STAGE_FLOATS;
+    const float* st = smem + slot * SF;
     if (!C.pre) mbar_wait(&Q.full[slot], (C.it / FNS) & 1);
     const V4 v = ld4(st + F_OFF_PT + K.toff);
     V4 vz4 = ld4(st + F_OFF_VZ + K.toff);
+    V4 bz4;
+    if (HB) bz4 = ld4(st + F_OFF_BZ + K.toff);
     warp_arrive(&Q.empty[slot]);
     C.pre = mbar_test(&Q.full[(C.it + 1) % FNS], ((C.it + 1) / FNS) & 1);
-    shift_push(C.pq, v);
-    vz4 = fused_vz(D, O, K, C, C.pq[0], C.pq[1], C.pq[2], C.pq[3], C.pq[4], C.pq[5], C.pq[6], C.pq[7], vz4, m - 4);
-    shift_push(C.wq, vz4);
+#pragma unroll
+    for (int n = 0; n < 7; ++n) C.pq[n] = C.pq[n + 1];
+    C.pq[7] = v;
+    const int kz = m - 4;                                            // planes z0 .. z0+2 are this item's own
+    vz4 = fused_vz<HB, true>(D, O, K, C.pq[0], C.pq[1], C.pq[2], C.pq[3], C.pq[4], C.pq[5], C.pq[6], C.pq[7], vz4, bz4, kz,
+                       K.zrow + (long long)kz * D.plane, K.active && kz >= z0 && kz < z1);
+#pragma unroll
+    for (int n = 0; n < 7; ++n) C.wq[n] = C.wq[n + 1];
+    C.wq[7] = vz4;
   }
-  // after lead-in 2 the rings are canonical for m = z0+6; one more rotation step puts the oldest entry at index 0 = R
-  if (XY) {
-    if (K.sx >= 0) { C.nvx = ldg4(D.psi[0][0][K.sx] + C.pox); C.npx = ldg4(D.psi[1][0][K.sx] + C.pox); }
-    if (K.sy >= 0) { C.nvy = ldg4(D.psi[0][1][K.sy] + C.poy); C.npy = ldg4(D.psi[1][1][K.sy] + C.poy); }
-  }
-  for (int k = z0; k < z1; ++k) fused_steady<7, XY>(D, O, smem, ebuf, Q, K, C, k);
-}
-
-__device__ __forceinline__ void fused_main(const DomainView& D, const OutSet& O, const float* smem, float* ebuf, const FusedBars& Q,
-                                           const TabCache& T, unsigned& it, unsigned& eit, int x0, int y0, int z0, int z1) {
-  const int tid = threadIdx.x;
-  MainConst K;
-  K.tx = tid & 15; K.ty = tid >> 4;
-  K.i = x0 + 4 * K.tx; K.j = y0 + K.ty;
-  K.z0 = z0; K.z1 = z1;
-  K.has_kc = D.kc != nullptr;
-  K.active = (K.i < D.nx) && (K.j < D.ny);
-  K.Bxy = K.active ? D.b0 : 0.f;
-  K.Bx3 = (K.i + 3 + D.ox) == D.gn[0] - 1 ? 0.f : K.Bxy;           // pinned last half node (R3)
-  K.By = (K.j + D.oy) == D.gn[1] - 1 ? 0.f : K.Bxy;
-  K.zrow = (long long)K.j * D.pitch + K.i;
-  K.boff = (K.ty + 7) * BW + 4 * K.tx + 8;                          // own float4 in the p box
-  K.toff = K.ty * TX + 4 * K.tx;                                    // own float4 in a plain tile
-  K.exo = K.ty * HW + 4 * K.tx + 4;                                 // own float4 in E.vx and in the vx x-halo tile
-  K.eyo = E_OFF_VY + (K.ty + 4) * TX + 4 * K.tx;                    // own float4 in E.vy
-  K.zl = D.ln[2][0];                                                // low z slab = local planes [0, zl)
-  K.zh = D.ln[2][1] > 0 ? D.ls[2][1] : 0x7fffffff;                  // high z slab = local planes [zh, nz)
-  const bool any_xy = touches(D, 0, x0, x0 + TX) || touches(D, 1, y0, y0 + TY);
-  K.sx = (any_xy && K.active) ? slab_side(D, 0, K.i) : -1;
-  K.sy = (any_xy && K.active) ? slab_side(D, 1, K.j) : -1;
-  K.stride_px = K.sx >= 0 ? (long long)D.ny * D.ln[0][K.sx] : 0;
-  K.stride_py = K.sy >= 0 ? (long long)D.ln[1][K.sy] * D.pitch : 0;
-  K.gi = K.i + D.ox; K.gj = K.j + D.oy;
-  K.T = &T;
-  MainCtx C;
-  C.it = it; C.eit = eit; C.pre = false;
-  C.pox = K.sx >= 0 ? psi_index(D, 0, K.sx, K.i, K.j, z0) : 0;
-  C.poy = K.sy >= 0 ? psi_index(D, 1, K.sy, K.i, K.j, z0) : 0;
-  const long long goff = K.zrow + (long long)z0 * D.plane;
-  C.gvx = O.f[1] + goff; C.gvy = O.f[2] + goff; C.gp = O.f[0] + goff;
-  C.gvz = O.f[3] + K.zrow + (long long)(z0 - 4) * D.plane;          // first vz plane computed is z0-4 (stored from z0 on)
-  if (any_xy) fused_main_item<true>(D, O, smem, ebuf, Q, K, C);
-  else fused_main_item<false>(D, O, smem, ebuf, Q, K, C);
-  it = C.it; eit = C.eit;
+  // now pq[n] = p_old[z0-1+n], wq[n] = vz_new[z0-5+n]: entry 0 of both rings is the oldest
+  if (XS && K.in_x) { C.nvx = ldg4(K.psi_in[0][0] + C.pox); C.npx = ldg4(K.psi_in[1][0] + C.pox); }
+  if (YS && K.in_y) { C.nvy = ldg4(K.psi_in[0][1] + C.poy); C.npy = ldg4(K.psi_in[1][1] + C.poy); }
+  // z range of the item = [z0, za) + [za, zb) + [zb, z1): only the outer two can touch a z slab (plane k or vz plane k+3)
+  const int za = min(max(K.zl, z0), z1), zb = min(max(K.zh - 3, za), z1);
+  fused_run<true, XS, YS, HB>(D, O, smem, ebuf, Q, T, K, C, z0, za);
+  fused_run<false, XS, YS, HB>(D, O, smem, ebuf, Q, T, K, C, za, zb);
+  fused_run<true, XS, YS, HB>(D, O, smem, ebuf, Q, T, K, C, zb, z1);
+  it_io = C.it; eit_io = C.eit;
 }
 
 // ---- halo warps: the redundantly computed ghost of the tile, never stored to global memory ----------------
 // Warp hw (0..3) computes vy_new on two of the rows y0-4..y0-1, y0+TY..y0+TY+2 (16 float4 units per row; the eighth
 // row slot is idle); warp 3 also computes vx_new on the strips x0-4..x0-1 and x0+TX..x0+TX+3 (rows y0..y0+TY-1).
-// Lane 0 of warp 0 is the TMA producer of the CTA.
-__device__ __forceinline__ void fused_halo(const TMaps& tm, const DomainView& D, float* smem, float* ebuf, const FusedBars& Q,
-                                           const TabCache& T, unsigned it,
+template <bool HB>
+__device__ __forceinline__ void fused_halo(const DomainView& D, float* smem, float* ebuf, const FusedBars& Q, const TabCache& T, unsigned it,
                                            unsigned eit, int hw, int x0, int y0, int z0, int z1) {
   const int lane = threadIdx.x & 31;
-  const bool has_kc = D.kc != nullptr;
+  constexpr int SF = f_stage_floats<HB>();
   // vy unit of this lane
   const int r = 2 * hw + (lane >> 4), c = lane & 15;
   const int jy = r < 4 ? y0 - 4 + r : y0 + TY + (r - 4), iy = x0 + 4 * c;
@@ -379,18 +442,20 @@ __device__ __forceinline__ void fused_halo(const TMaps& tm, const DomainView& D,
       if (sy >= 0) npsy = ldg4(D.psi[0][1][sy] + poy + stride_py);
       if (sx >= 0) npsx = ldg4(D.psi[0][0][sx] + pox + stride_px);
     }
-    const float* st = smem + slot * F_STAGE_FLOATS;
+    const float* st = smem + slot * SF;
     mbar_wait(&Q.full[slot], (it / FNS) & 1);
-    V4 dyv, vy4, dxv, vx4;
+    V4 dyv, vy4, dxv, vx4, by4, bx4;
     if (out) {
       const float* rw = st + boff_y;
       dyv = diff_8(ld4(rw + BW), ld4(rw), ld4(rw + 2 * BW), ld4(rw - BW), ld4(rw + 3 * BW), ld4(rw - 2 * BW), ld4(rw + 4 * BW),
                    ld4(rw - 3 * BW));
       vy4 = ld4(st + F_OFF_VY + eyo);
+      if (HB) by4 = ld4(st + F_OFF_BY + eyo);
       if (do_x) {
         const float* rx = st + boff_x;
         dxv = diff_x<true>(ld4(rx - 4), ld4(rx), ld4(rx + 4));
         vx4 = ld4(st + F_OFF_VX + exo);
+        if (HB) bx4 = ld4(st + F_OFF_BX + exo);
       }
     }
     warp_arrive(&Q.empty[slot]);
@@ -399,13 +464,23 @@ __device__ __forceinline__ void fused_halo(const TMaps& tm, const DomainView& D,
         cpml4s(dyv, psy, T.y[0][0][rr], T.y[0][1][rr], T.y[0][2][rr]);
         poy += stride_py;
       }
-      vy4 = upd4(vy4, By, By, By, dyv);
+      if (HB) {
+#pragma unroll
+        for (int e = 0; e < 4; ++e) vy4.v[e] = upd(vy4.v[e], By == 0.f ? 0.f : by4.v[e], dyv.v[e]);
+      } else {
+        vy4 = upd4(vy4, By, By, By, dyv);
+      }
       if (do_x) {
         if (sx >= 0) {
           cpml4(dxv, psx, ld4(T.x[0][0] + xcol), ld4(T.x[0][1] + xcol), ld4(T.x[0][2] + xcol));
           pox += stride_px;
         }
-        vx4 = upd4(vx4, Bvx, Bvx, Bx3, dxv);
+        if (HB) {
+#pragma unroll
+          for (int e = 0; e < 4; ++e) vx4.v[e] = upd(vx4.v[e], (Bvx == 0.f || (e == 3 && Bx3 == 0.f)) ? 0.f : bx4.v[e], dxv.v[e]);
+        } else {
+          vx4 = upd4(vx4, Bvx, Bvx, Bx3, dxv);
+        }
       }
       const unsigned eb = eit & 1;
       float* E = ebuf + eb * E_FLOATS;
@@ -420,11 +495,12 @@ __device__ __forceinline__ void fused_halo(const TMaps& tm, const DomainView& D,
   }
 }
 
+template <bool HB>
 __global__ void __launch_bounds__(FNT, 1) step_fused(const __grid_constant__ TMaps tm, const __grid_constant__ DomainView D,
                                                      const __grid_constant__ OutSet O, const __grid_constant__ Sched S) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   float* smem = reinterpret_cast<float*>(smem_raw);
-  float* ebuf = smem + FNS * F_STAGE_FLOATS;
+  float* ebuf = smem + FNS * f_stage_floats<HB>();
   __shared__ __align__(8) uint64_t bars[2 * FNS + 2];
   __shared__ int s_item;
   __shared__ __align__(16) TabCache tabc;
@@ -439,20 +515,24 @@ __global__ void __launch_bounds__(FNT, 1) step_fused(const __grid_constant__ TMa
   const int warp = threadIdx.x >> 5;
   unsigned it = 0, eit = 0;
   int x0, y0, z0, z1;
-  // The two roles never share code after this point, so each is compiled against its own register budget: the two main
-  // warpgroups take the registers the halo warpgroup gives up (3 warps per SM sub-partition: 2 x 216 + 72 <= 512).
+  // The roles never share code after this point, so each is compiled against its own register budget: the two main
+  // warpgroups take the registers the halo and producer warpgroups give up (2 x 200 + 80 + 32 <= 512 per sub-partition lane).
   if (warp < FW_MAIN) {
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(F_REGS_MAIN));
     while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) {
       fill_tab_cache(D, tabc, x0, y0);
-      fused_main(D, O, smem, ebuf, Q, tabc, it, eit, x0, y0, z0, z1);
+      const bool xs = touches(D, 0, x0, x0 + TX), ys = touches(D, 1, y0, y0 + TY);      // block-uniform
+      if (!xs && !ys) fused_main_item<false, false, HB>(D, O, smem, ebuf, Q, tabc, it, eit, x0, y0, z0, z1);
+      else if (xs && !ys) fused_main_item<true, false, HB>(D, O, smem, ebuf, Q, tabc, it, eit, x0, y0, z0, z1);
+      else if (!xs) fused_main_item<false, true, HB>(D, O, smem, ebuf, Q, tabc, it, eit, x0, y0, z0, z1);
+      else fused_main_item<true, true, HB>(D, O, smem, ebuf, Q, tabc, it, eit, x0, y0, z0, z1);
     }
   } else if (warp < FNW) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(F_REGS_HALO));
     while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) {
       fill_tab_cache(D, tabc, x0, y0);
-      fused_halo(tm, D, smem, ebuf, Q, tabc, it, eit, warp - FW_MAIN, x0, y0, z0, z1);
-      it += z1 - z0 + 14;
+      fused_halo<HB>(D, smem, ebuf, Q, tabc, it, eit, warp - FW_MAIN, x0, y0, z0, z1);
+      it += z1 - z0 + F_LEAD;
       eit += z1 - z0;
     }
   } else {
@@ -460,12 +540,12 @@ __global__ void __launch_bounds__(FNT, 1) step_fused(const __grid_constant__ TMa
     const bool has_kc = D.kc != nullptr;
     const bool producer = threadIdx.x == FNW * 32;
     while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) {
-      const int niter = z1 - z0 + 14;
+      const int niter = z1 - z0 + F_LEAD;
       if (producer) {
         for (int s = 0; s < niter; ++s) {
           const unsigned slot = (it + s) % FNS;
           if (s >= FNS) mbar_wait(&Q.empty[slot], ((it + s - FNS) / FNS) & 1);      // every consumer warp released the stage
-          fused_issue(tm, smem, Q.full, slot, z0 - 7 + s, x0, y0, z0, has_kc);
+          fused_issue<HB>(tm, smem, Q.full, slot, z0 - 7 + s, x0, y0, z0, has_kc);
         }
       }
       it += niter;

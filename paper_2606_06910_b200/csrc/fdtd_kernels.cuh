@@ -21,91 +21,130 @@ namespace fdtd {
 #define FDTD_C3 (49.0f / 5120.0f)
 #define FDTD_C4 (-5.0f / 7168.0f)
 
-// One domain (the whole grid, or one in-HBM subdomain with its ghost cells) as the kernels see it.
-struct DomainView {
+// One domain (the whole grid, or one in-HBM subdomain with its ghost cells) as the kernels see it.  T = float is the
+// product path; T = double is the verification precision: state and arithmetic in double, every coefficient
+// (weights, CPML tables, K dt/dx, dt/(rho_bar dx), wavelets) the same fp32 number as in the fp32 path.
+template <class T>
+struct DomainViewT {
+  typedef T real;
   int nx, ny, nz;          // local extents (ghost cells included)
-  int pitch;               // floats per x row (multiple of 8; columns >= nx are kept zero)
+  int pitch;               // elements per x row (multiple of 8; columns >= nx are kept zero)
   long long plane;         // pitch * ny
   int ox, oy, oz;          // global index of local (0,0,0)
   int gn[3];               // global total-grid extents
   int periodic;
-  float* f[4];             // p, vx, vy, vz
+  T* f[4];                 // p, vx, vy, vz
   const float* kc;         // K dt/dx per node (local layout) or nullptr -> kc0
   float kc0, b0;           // homogeneous K dt/dx and dt/(rho dx)
   const float* bq[3];      // dt/(rho_bar dx) at the half nodes of vx, vy, vz (local layout) or nullptr -> b0 (R6)
   int ls[3][2], ln[3][2];  // CPML storage slabs in LOCAL indices: [axis][side] start, count (0 = none)
-  float* psi[2][3][2];     // [family 0 = psi_v, 1 = psi_p][axis][side], slab-local
+  T* psi[2][3][2];         // [family 0 = psi_v, 1 = psi_p][axis][side], slab-local
   const float* tab[2][3][3];  // [family][axis][a, b, 1/kappa], indexed by GLOBAL index along the axis
 };
+typedef DomainViewT<float> DomainView;
 
 // ---------------------------------------------------------------- arithmetic (identical in every kernel)
 // D = sum_l c_l (hi_l - lo_l), accumulated l = 1..4 (P:38 in the staggered reading R1).
+// Every product and every sum is rounded on its own, in the order of the recurrence as written:
+// no fused multiply-add.  The result therefore has the bits of the plain evaluation — the fp32 oracle's — and parity is
+// exact instead of "within rounding" (an FMA chain drifts from it by 1e-4 of the final field over 500 steps near a point
+// source, where the velocity has cancelled from 300 times its final size; measured cost of the separate roundings: 2 %,
+// the kernels are bound by shared-memory and HBM bandwidth, not by arithmetic issue).
+__device__ __forceinline__ float mad(float a, float b, float c) { return __fadd_rn(__fmul_rn(a, b), c); }
+// Packed fp32x2 (sm_100a FADD2 / FMUL2): two independent IEEE operations per instruction.  ptxas contracts a packed
+// multiply into a packed add that consumes it (FFMA2) whatever the rounding modifiers say, so every product that feeds a
+// sum is formed by two scalar FMULs; only the sums and differences are packed.
+__device__ __forceinline__ float2 mul2(float2 a, float2 b) { return make_float2(__fmul_rn(a.x, b.x), __fmul_rn(a.y, b.y)); }
+__device__ __forceinline__ float2 mad2(float2 a, float2 b, float2 c) { return __fadd2_rn(mul2(a, b), c); }
 __device__ __forceinline__ float stag_diff(float h1, float l1, float h2, float l2, float h3, float l3, float h4, float l4) {
   float d = __fmul_rn(FDTD_C1, __fsub_rn(h1, l1));
-  d = __fmaf_rn(FDTD_C2, __fsub_rn(h2, l2), d);
-  d = __fmaf_rn(FDTD_C3, __fsub_rn(h3, l3), d);
-  d = __fmaf_rn(FDTD_C4, __fsub_rn(h4, l4), d);
+  d = mad(FDTD_C2, __fsub_rn(h2, l2), d);
+  d = mad(FDTD_C3, __fsub_rn(h3, l3), d);
+  d = mad(FDTD_C4, __fsub_rn(h4, l4), d);
   return d;
 }
 // psi <- b psi + a d ; returns d/kappa + psi (update-then-use R10).
 __device__ __forceinline__ float cpml_apply(float d, float& psi, float a, float b, float ik) {
-  psi = __fmaf_rn(b, psi, __fmul_rn(a, d));
-  return __fmaf_rn(d, ik, psi);
+  psi = mad(b, psi, __fmul_rn(a, d));
+  return mad(d, ik, psi);
 }
-__device__ __forceinline__ float upd(float f, float coef, float d) { return __fmaf_rn(-coef, d, f); }
+__device__ __forceinline__ float upd(float f, float coef, float d) { return mad(-coef, d, f); }
+// the same sequences in double (verification precision): products and sums rounded separately here too
+__device__ __forceinline__ double mad(double a, double b, double c) { return __dadd_rn(__dmul_rn(a, b), c); }
+__device__ __forceinline__ double stag_diff(double h1, double l1, double h2, double l2, double h3, double l3, double h4, double l4) {
+  double d = __dmul_rn((double)FDTD_C1, __dsub_rn(h1, l1));
+  d = mad((double)FDTD_C2, __dsub_rn(h2, l2), d);
+  d = mad((double)FDTD_C3, __dsub_rn(h3, l3), d);
+  d = mad((double)FDTD_C4, __dsub_rn(h4, l4), d);
+  return d;
+}
+__device__ __forceinline__ double cpml_apply(double d, double& psi, double a, double b, double ik) {
+  psi = mad(b, psi, __dmul_rn(a, d));
+  return mad(d, ik, psi);
+}
+__device__ __forceinline__ double upd(double f, double coef, double d) { return mad(-coef, d, f); }
+__device__ __forceinline__ float add3(float a, float b, float c) { return __fadd_rn(__fadd_rn(a, b), c); }
+__device__ __forceinline__ double add3(double a, double b, double c) { return __dadd_rn(__dadd_rn(a, b), c); }
 
 // psi slab addressing (slab-local storage).
-__device__ __forceinline__ long long psi_index(const DomainView& D, int axis, int side, int i, int j, int k) {
+template <class V>
+__device__ __forceinline__ long long psi_index(const V& D, int axis, int side, int i, int j, int k) {
   if (axis == 0) return ((long long)k * D.ny + j) * D.ln[0][side] + (i - D.ls[0][side]);
   if (axis == 1) return ((long long)k * D.ln[1][side] + (j - D.ls[1][side])) * D.pitch + i;
   return ((long long)(k - D.ls[2][side]) * D.ny + j) * D.pitch + i;
 }
 // which storage slab (0 low, 1 high, -1 none) holds local index v of this axis
-__device__ __forceinline__ int slab_side(const DomainView& D, int axis, int v) {
+template <class V>
+__device__ __forceinline__ int slab_side(const V& D, int axis, int v) {
   if (D.ln[axis][0] > 0 && v >= D.ls[axis][0] && v < D.ls[axis][0] + D.ln[axis][0]) return 0;
   if (D.ln[axis][1] > 0 && v >= D.ls[axis][1] && v < D.ls[axis][1] + D.ln[axis][1]) return 1;
   return -1;
 }
 
 // ---------------------------------------------------------------- reference kernels (one thread per point)
-__device__ __forceinline__ float rd_ref(const DomainView& D, const float* __restrict__ a, int i, int j, int k) {
+template <class V>
+__device__ __forceinline__ typename V::real rd_ref(const V& D, const typename V::real* __restrict__ a, int i, int j, int k) {
   if (D.periodic) {
     i = (i % D.nx + D.nx) % D.nx; j = (j % D.ny + D.ny) % D.ny; k = (k % D.nz + D.nz) % D.nz;
   } else if (i < 0 || i >= D.nx || j < 0 || j >= D.ny || k < 0 || k >= D.nz) {
-    return 0.0f;
+    return 0;
   }
   return a[(long long)k * D.plane + (long long)j * D.pitch + i];
 }
 
-__global__ void __launch_bounds__(256) update_v_ref(DomainView D) {
+template <class V>
+__global__ void __launch_bounds__(256) update_v_ref(V D) {
+  typedef typename V::real T;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
   const int k = blockIdx.z;
   if (i >= D.nx || j >= D.ny || k >= D.nz) return;
   const long long q = (long long)k * D.plane + (long long)j * D.pitch + i;
-  const float* p = D.f[0];
+  const T* p = D.f[0];
   const int g[3] = {i + D.ox, j + D.oy, k + D.oz};
   const int loc[3] = {i, j, k};
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
     if (!D.periodic && g[a] == D.gn[a] - 1) continue;   // pinned last half node (R3)
     const int ex = a == 0, ey = a == 1, ez = a == 2;
-    float d = stag_diff(rd_ref(D, p, i + ex, j + ey, k + ez), rd_ref(D, p, i, j, k),
-                        rd_ref(D, p, i + 2 * ex, j + 2 * ey, k + 2 * ez), rd_ref(D, p, i - ex, j - ey, k - ez),
-                        rd_ref(D, p, i + 3 * ex, j + 3 * ey, k + 3 * ez), rd_ref(D, p, i - 2 * ex, j - 2 * ey, k - 2 * ez),
-                        rd_ref(D, p, i + 4 * ex, j + 4 * ey, k + 4 * ez), rd_ref(D, p, i - 3 * ex, j - 3 * ey, k - 3 * ez));
+    T d = stag_diff(rd_ref(D, p, i + ex, j + ey, k + ez), rd_ref(D, p, i, j, k),
+                    rd_ref(D, p, i + 2 * ex, j + 2 * ey, k + 2 * ez), rd_ref(D, p, i - ex, j - ey, k - ez),
+                    rd_ref(D, p, i + 3 * ex, j + 3 * ey, k + 3 * ez), rd_ref(D, p, i - 2 * ex, j - 2 * ey, k - 2 * ez),
+                    rd_ref(D, p, i + 4 * ex, j + 4 * ey, k + 4 * ez), rd_ref(D, p, i - 3 * ex, j - 3 * ey, k - 3 * ez));
     const int side = slab_side(D, a, loc[a]);
     if (side >= 0) {
-      float* ps = D.psi[0][a][side] + psi_index(D, a, side, i, j, k);
-      float s = *ps;
-      d = cpml_apply(d, s, D.tab[0][a][0][g[a]], D.tab[0][a][1][g[a]], D.tab[0][a][2][g[a]]);
+      T* ps = D.psi[0][a][side] + psi_index(D, a, side, i, j, k);
+      T s = *ps;
+      d = cpml_apply(d, s, (T)D.tab[0][a][0][g[a]], (T)D.tab[0][a][1][g[a]], (T)D.tab[0][a][2][g[a]]);
       *ps = s;
     }
-    D.f[1 + a][q] = upd(D.f[1 + a][q], D.bq[a] ? D.bq[a][q] : D.b0, d);
+    D.f[1 + a][q] = upd(D.f[1 + a][q], (T)(D.bq[a] ? D.bq[a][q] : D.b0), d);
   }
 }
 
-__global__ void __launch_bounds__(256) update_p_ref(DomainView D) {
+template <class V>
+__global__ void __launch_bounds__(256) update_p_ref(V D) {
+  typedef typename V::real T;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
   const int k = blockIdx.z;
@@ -113,26 +152,26 @@ __global__ void __launch_bounds__(256) update_p_ref(DomainView D) {
   const long long q = (long long)k * D.plane + (long long)j * D.pitch + i;
   const int g[3] = {i + D.ox, j + D.oy, k + D.oz};
   const int loc[3] = {i, j, k};
-  float dd[3];
+  T dd[3];
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
-    const float* v = D.f[1 + a];
+    const T* v = D.f[1 + a];
     const int ex = a == 0, ey = a == 1, ez = a == 2;
-    float d = stag_diff(rd_ref(D, v, i, j, k), rd_ref(D, v, i - ex, j - ey, k - ez),
-                        rd_ref(D, v, i + ex, j + ey, k + ez), rd_ref(D, v, i - 2 * ex, j - 2 * ey, k - 2 * ez),
-                        rd_ref(D, v, i + 2 * ex, j + 2 * ey, k + 2 * ez), rd_ref(D, v, i - 3 * ex, j - 3 * ey, k - 3 * ez),
-                        rd_ref(D, v, i + 3 * ex, j + 3 * ey, k + 3 * ez), rd_ref(D, v, i - 4 * ex, j - 4 * ey, k - 4 * ez));
+    T d = stag_diff(rd_ref(D, v, i, j, k), rd_ref(D, v, i - ex, j - ey, k - ez),
+                    rd_ref(D, v, i + ex, j + ey, k + ez), rd_ref(D, v, i - 2 * ex, j - 2 * ey, k - 2 * ez),
+                    rd_ref(D, v, i + 2 * ex, j + 2 * ey, k + 2 * ez), rd_ref(D, v, i - 3 * ex, j - 3 * ey, k - 3 * ez),
+                    rd_ref(D, v, i + 3 * ex, j + 3 * ey, k + 3 * ez), rd_ref(D, v, i - 4 * ex, j - 4 * ey, k - 4 * ez));
     const int side = slab_side(D, a, loc[a]);
     if (side >= 0) {
-      float* ps = D.psi[1][a][side] + psi_index(D, a, side, i, j, k);
-      float s = *ps;
-      d = cpml_apply(d, s, D.tab[1][a][0][g[a]], D.tab[1][a][1][g[a]], D.tab[1][a][2][g[a]]);
+      T* ps = D.psi[1][a][side] + psi_index(D, a, side, i, j, k);
+      T s = *ps;
+      d = cpml_apply(d, s, (T)D.tab[1][a][0][g[a]], (T)D.tab[1][a][1][g[a]], (T)D.tab[1][a][2][g[a]]);
       *ps = s;
     }
     dd[a] = d;
   }
-  const float kc = D.kc ? D.kc[q] : D.kc0;
-  D.f[0][q] = upd(D.f[0][q], kc, __fadd_rn(__fadd_rn(dd[0], dd[1]), dd[2]));
+  const T kc = (T)(D.kc ? D.kc[q] : D.kc0);
+  D.f[0][q] = upd(D.f[0][q], kc, add3(dd[0], dd[1], dd[2]));
 }
 
 // ---------------------------------------------------------------- TMA / mbarrier primitives (inline PTX)
@@ -220,6 +259,8 @@ struct TMaps {
   CUtensorMap vy_halo;    // vy, box TX x PH   (update_p)
   CUtensorMap tile[5];    // p, vx, vy, vz, kc with box TX x TY
   CUtensorMap p_box;      // p,  box (TX+16) x (TY+14)   (step_fused)
+  CUtensorMap bq_halo[2]; // dt/(rho_bar dx) of vx, box HW x TY; of vy, box TX x PH   (step_fused<true>)
+  CUtensorMap bq_tile;    // dt/(rho_bar dx) of vz, box TX x TY                         (step_fused<true>)
 };
 
 // Work decomposition of one launch (same for both sub-updates of a domain).
@@ -253,15 +294,13 @@ __device__ __forceinline__ V4 diff_x(const V4& l, const V4& c, const V4& r) {
   }
   return d;
 }
-// Packed fp32x2 forms (sm_100a FADD2 / FMUL2 / FFMA2: two independent IEEE operations per instruction, so the bits
-// are those of the scalar sequence; they halve the issue slots of the arithmetic).
 __device__ __forceinline__ float2 pk(float a, float b) { return make_float2(a, b); }
 __device__ __forceinline__ float2 sub2(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
 __device__ __forceinline__ float2 stag_diff2(float2 h1, float2 l1, float2 h2, float2 l2, float2 h3, float2 l3, float2 h4, float2 l4) {
-  float2 d = __fmul2_rn(pk(FDTD_C1, FDTD_C1), sub2(h1, l1));
-  d = __ffma2_rn(pk(FDTD_C2, FDTD_C2), sub2(h2, l2), d);
-  d = __ffma2_rn(pk(FDTD_C3, FDTD_C3), sub2(h3, l3), d);
-  d = __ffma2_rn(pk(FDTD_C4, FDTD_C4), sub2(h4, l4), d);
+  float2 d = mul2(pk(FDTD_C1, FDTD_C1), sub2(h1, l1));
+  d = mad2(pk(FDTD_C2, FDTD_C2), sub2(h2, l2), d);
+  d = mad2(pk(FDTD_C3, FDTD_C3), sub2(h3, l3), d);
+  d = mad2(pk(FDTD_C4, FDTD_C4), sub2(h4, l4), d);
   return d;
 }
 __device__ __forceinline__ float2 lo2(const V4& a) { return make_float2(a.v[0], a.v[1]); }
@@ -274,17 +313,17 @@ __device__ __forceinline__ V4 diff_8(const V4& h1, const V4& l1, const V4& h2, c
 }
 // f - coef d for four points, coefficients (c01, c01, c2, c3)
 __device__ __forceinline__ V4 upd4(const V4& f, float c01, float c2, float c3, const V4& d) {
-  return join2(__ffma2_rn(pk(-c01, -c01), lo2(d), lo2(f)), __ffma2_rn(pk(-c2, -c3), hi2(d), hi2(f)));
+  return join2(mad2(pk(-c01, -c01), lo2(d), lo2(f)), mad2(pk(-c2, -c3), hi2(d), hi2(f)));
 }
 __device__ __forceinline__ void cpml4(V4& d, V4& ps, const V4& a, const V4& b, const V4& ik) {
-  const float2 p0 = __ffma2_rn(lo2(b), lo2(ps), __fmul2_rn(lo2(a), lo2(d))), p1 = __ffma2_rn(hi2(b), hi2(ps), __fmul2_rn(hi2(a), hi2(d)));
-  d = join2(__ffma2_rn(lo2(d), lo2(ik), p0), __ffma2_rn(hi2(d), hi2(ik), p1));
+  const float2 p0 = mad2(lo2(b), lo2(ps), mul2(lo2(a), lo2(d))), p1 = mad2(hi2(b), hi2(ps), mul2(hi2(a), hi2(d)));
+  d = join2(mad2(lo2(d), lo2(ik), p0), mad2(hi2(d), hi2(ik), p1));
   ps = join2(p0, p1);
 }
 __device__ __forceinline__ void cpml4s(V4& d, V4& ps, float a, float b, float ik) {
   const float2 a2 = pk(a, a), b2 = pk(b, b), k2 = pk(ik, ik);
-  const float2 p0 = __ffma2_rn(b2, lo2(ps), __fmul2_rn(a2, lo2(d))), p1 = __ffma2_rn(b2, hi2(ps), __fmul2_rn(a2, hi2(d)));
-  d = join2(__ffma2_rn(lo2(d), k2, p0), __ffma2_rn(hi2(d), k2, p1));
+  const float2 p0 = mad2(b2, lo2(ps), mul2(a2, lo2(d))), p1 = mad2(b2, hi2(ps), mul2(a2, hi2(d)));
+  d = join2(mad2(lo2(d), k2, p0), mad2(hi2(d), k2, p1));
   ps = join2(p0, p1);
 }
 
@@ -649,13 +688,16 @@ __global__ void __launch_bounds__(NT, 2) update_p_tiled(const __grid_constant__ 
 // p[src_s] += w_s[n] for every source (R14).  The step index n is kept on the host and passed in, so steps taken
 // before fdtd_set_sources count too.  Sources that share a node are added by the first of them, one after the other in
 // source order — the order of the recurrence (oracle: a plain loop over the sources), and no lost update.
-struct SourceView {
+template <class T>
+struct SourceViewT {
   int n, len;
   const long long* offset;   // flat element offset of each source in its domain's p array, or -1 if not held
-  float* p;
+  T* p;
   const float* wav;
 };
-__global__ void inject_sources(SourceView S, long long n) {
+typedef SourceViewT<float> SourceView;
+template <class T>
+__global__ void inject_sources(SourceViewT<T> S, long long n) {
   if (n >= S.len) return;
   for (int s = threadIdx.x; s < S.n; s += blockDim.x) {
     const long long off = S.offset[s];
@@ -663,9 +705,9 @@ __global__ void inject_sources(SourceView S, long long n) {
     bool first = true;
     for (int t = 0; t < s; ++t) first = first && S.offset[t] != off;
     if (!first) continue;
-    float v = S.p[off];
+    T v = S.p[off];
     for (int t = s; t < S.n; ++t)
-      if (S.offset[t] == off) v = __fadd_rn(v, S.wav[(long long)t * S.len + n]);
+      if (S.offset[t] == off) v = v + (T)S.wav[(long long)t * S.len + n];      // one rounded addition per source
     S.p[off] = v;
   }
 }
@@ -686,7 +728,8 @@ __device__ __forceinline__ uint64_t splitmix64(uint64_t x) {
   return x ^ (x >> 31);
 }
 // Counter-based synthetic initial state: value depends on the GLOBAL index only.
-__global__ void fill_hash_kernel(DomainView D, int which, uint64_t seed, float scale) {
+template <class V>
+__global__ void fill_hash_kernel(V D, int which, uint64_t seed, float scale) {
   const long long n = (long long)D.nx * D.ny * D.nz;
   for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
     const int i = (int)(t % D.nx);
@@ -699,21 +742,23 @@ __global__ void fill_hash_kernel(DomainView D, int which, uint64_t seed, float s
   }
 }
 
-__global__ void absmax_kernel(DomainView D, int which, int lx, int ly, int lz, int sx, int sy, int sz, unsigned int* out) {
+template <class V>
+__global__ void absmax_kernel(V D, int which, int lx, int ly, int lz, int sx, int sy, int sz, unsigned int* out) {
   const long long n = (long long)sx * sy * sz;
   float m = 0.f;
   for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
     const int i = (int)(t % sx);
     const long long r = t / sx;
     const int j = (int)(r % sy), k = (int)(r / sy);
-    m = fmaxf(m, fabsf(D.f[which][(long long)(k + lz) * D.plane + (long long)(j + ly) * D.pitch + (i + lx)]));
+    m = fmaxf(m, fabsf((float)D.f[which][(long long)(k + lz) * D.plane + (long long)(j + ly) * D.pitch + (i + lx)]));
   }
   for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
   if ((threadIdx.x & 31) == 0) atomicMax(out, __float_as_uint(m));   // non-negative floats order like unsigned ints
 }
 
 // Expand one slab-local psi array into a full-volume scratch array (debug / parity of the recursion).
-__global__ void expand_psi_kernel(DomainView D, int fam, int axis, float* out /* nx*ny*nz packed */) {
+template <class V>
+__global__ void expand_psi_kernel(V D, int fam, int axis, typename V::real* out /* nx*ny*nz packed */) {
   const long long n = (long long)D.nx * D.ny * D.nz;
   for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
     const int i = (int)(t % D.nx);
@@ -721,7 +766,7 @@ __global__ void expand_psi_kernel(DomainView D, int fam, int axis, float* out /*
     const int j = (int)(r % D.ny), k = (int)(r / D.ny);
     const int loc[3] = {i, j, k};
     const int side = slab_side(D, axis, loc[axis]);
-    out[t] = side >= 0 ? D.psi[fam][axis][side][psi_index(D, axis, side, i, j, k)] : 0.f;
+    out[t] = side >= 0 ? D.psi[fam][axis][side][psi_index(D, axis, side, i, j, k)] : 0;
   }
 }
 

@@ -5,10 +5,10 @@
 Splits the 512^3 + 20-cell-CPML grid into 1x2x2 in-HBM subdomains with ghost width g and m sub-updates between halo
 exchanges (g >= 4 m; (8,2) is the paper's s = 1, (16,4) its s = 2, (32,8) its s = 4), times it against the monolithic
 kernel and reports the redundant ghost compute (points updated / points owned) and the exchange share.  Prints one
-JSON object per line.  --layouts adds the other decompositions the library supports at (g, m) = (8, 2): slab-z 1x1x4
-(P:76), slab-y 1x4x1 and 1x4x2; block-xy 2x2x1 would split the contiguous x axis and is not supported, which is
-the paper's own conclusion about that layout.  --fused runs the subdomains with the single-pass step
-(two sub-updates per launch, so m is even)."""
+JSON object per line.  --layouts runs the three four-subdomain layouts of the paper's Table 5 at
+(g, m) = (8, 2) — slab-z 1x1x4, block-xy 2x2x1 (its halo cuts the contiguous x axis: g-wide column blocks), pencil-yz
+1x2x2 — plus slab-y 1x4x1 and 1x4x2, with the halo-exchange time split out, so that the ordering of Table 5 can be
+compared by halo cost.  --fused runs the subdomains with the single-pass step (two sub-updates per launch, so m is even)."""
 import argparse
 import json
 
@@ -47,16 +47,18 @@ def main():
                       "kernels_ms": prof0}))
     own = w.total[1] // 2
     if a.layouts:
-        for name, dec in (("slab-z 1x1x4", (1, 1, 4)), ("slab-y 1x4x1", (1, 4, 1)), ("pencil-yz 1x2x2", (1, 2, 2)), ("1x4x2", (1, 4, 2))):
+        for name, dec in (("slab-z 1x1x4", (1, 1, 4)), ("block-xy 2x2x1", (2, 2, 1)), ("pencil-yz 1x2x2", (1, 2, 2)), ("slab-y 1x4x1", (1, 4, 1)),
+                          ("1x4x2", (1, 4, 2))):
             g, m = 8, 2
             ms, prof = run(w, a.steps, decomp=dec, ghost=g, substeps=m, kernel=kern)
             upd = 1.0                       # points updated / points owned: edge subdomains carry one ghost side, inner ones two
-            for ax in (1, 2):
+            for ax in (0, 1, 2):
                 d, o = dec[ax], w.total[ax] // dec[ax]
                 if d > 1:
                     upd *= (2 * (o + g) + (d - 2) * (o + 2 * g)) / (o * d)
             print(json.dumps({"layout": name, "ghost": g, "substeps_per_exchange": m, "ms_per_step": ms, "Mpts_s": pts / ms / 1e3,
-                              "vs_monolithic": ms0 / ms, "points_updated_per_owned": upd, "kernels_ms": prof}))
+                              "vs_monolithic": ms0 / ms, "points_updated_per_owned": upd, "exchange_ms": prof["exchange"],
+                              "exchange_share": prof["exchange"] / sum(prof.values()), "kernels_ms": prof}))
         return
     for g, m in ((4, 1), (8, 2), (16, 4), (32, 8), (16, 2), (32, 4)):
         if a.fused and m % 2:

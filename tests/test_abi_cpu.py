@@ -20,7 +20,7 @@ def lib():
 def _declared():
     src = open(os.path.join(ROOT, "include", "fdtd_b200.h")).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(fdtd_[a-z_]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(fdtd_[a-z0-9_]+)\s*\(", src)))
 
 
 def test_library_exports_every_declared_symbol(lib):
@@ -52,7 +52,11 @@ def test_workspace_bytes_and_validation():
     assert B.fdtd_workspace_bytes(bad) == 0 and "n_interior" in B.last_error()
     bad = B.make_params((32,) * 3, (8,) * 6, decomp=(1, 2, 2), ghost=4, substeps=2)          # g < 4 m
     assert B.fdtd_workspace_bytes(bad) == 0 and "ghost" in B.last_error()
-    bad = B.make_params((32,) * 3, decomp=(2, 1, 1), ghost=8, substeps=2)
+    ok = B.make_params((32,) * 3, decomp=(2, 1, 1), ghost=8, substeps=2)                     # an x cut (block-xy)
+    assert B.fdtd_workspace_bytes(ok) > 0
+    bad = B.make_params((32,) * 3, decomp=(2, 1, 1), ghost=6, substeps=1)                    # ... needs float4-aligned ghosts
+    assert B.fdtd_workspace_bytes(bad) == 0 and "multiples of 4" in B.last_error()
+    bad = B.make_params((24,) * 3, (8,) * 6, decomp=(2, 1, 1), ghost=8, substeps=2)         # ... and room beside the x layers
     assert B.fdtd_workspace_bytes(bad) == 0
     bad = B.make_params((32,) * 3, dt=0.0)
     assert B.fdtd_workspace_bytes(bad) == 0

@@ -1,7 +1,11 @@
 """GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element.
 
 Tolerance (BASELINE.json north_star, reading R17): max|delta| / max|oracle| <= 1e-4 per field, fp32.  The fp64 oracle
-(fed the same fp32 inputs) arbitrates (R18): the GPU and the fp32 oracle must each be within 1e-4 of it."""
+(fed the same fp32 inputs) arbitrates (R18): the GPU and the fp32 oracle must each be within 1e-4 of it.
+
+The kernels round every product and every sum on its own, in the order of the recurrence (no fused multiply-add, reading
+R25), so against the fp32 oracle the bar here is stricter than the tolerance: the same bits, in every field and every
+CPML memory variable, for all three kernel families."""
 import math
 
 import numpy as np
@@ -26,6 +30,15 @@ def B():
 def rel(a, b):
     s = np.abs(b).max()
     return float(np.abs(a.astype(np.float64) - b).max() / (s if s > 0 else 1.0))
+
+
+def assert_parity(g, r, tag):
+    """Within BASELINE's tolerance of the fp32 oracle, and bit for bit equal to it."""
+    e = rel(g, r)
+    assert e <= TOL, (tag, e)
+    r32 = np.ascontiguousarray(r, np.float32)
+    diff = int((np.ascontiguousarray(g).view(np.uint32) != r32.view(np.uint32)).sum())
+    assert diff == 0, (tag, "%d words differ from the fp32 oracle, max |delta| %.3e" % (diff, float(np.abs(g - r32).max())))
 
 
 def oracle_for(w, fp64=False):
@@ -60,11 +73,11 @@ def test_config1_full_parity(B, kernel):
     o64.step(w.steps)
     for f in range(4):
         g, r32, r64 = sim.get_field(f), o32.get(f), o64.get(f)
-        assert rel(g, r32) <= TOL, (f, rel(g, r32))
+        assert_parity(g, r32, f)
         assert rel(g, r64) <= TOL and rel(r32, r64) <= TOL
     for q in range(6):
         g, r = sim.get_psi(q), o32.get(4 + q)
-        assert rel(g, r) <= TOL, (q, rel(g, r))
+        assert_parity(g, r, ("psi", q))
     assert sim.launch_count() >= 2 * w.steps
     sim.destroy()
 
@@ -100,9 +113,9 @@ def test_random_state_ragged_parity(B, kernel, shape, cpml):
     sim.step(6)
     o.step(6)
     for f in range(4):
-        assert rel(sim.get_field(f), o.get(f)) <= TOL, (f, rel(sim.get_field(f), o.get(f)))
+        assert_parity(sim.get_field(f), o.get(f), f)
     for q in range(6):
-        assert rel(sim.get_psi(q), o.get(4 + q)) <= TOL, q
+        assert_parity(sim.get_psi(q), o.get(4 + q), ("psi", q))
     sim.destroy()
 
 
@@ -174,9 +187,9 @@ def test_paper_cpml_parameter_set_parity(B, kernel):
     sim.step(40)
     o.step(40)
     for f in range(4):
-        assert rel(sim.get_field(f), o.get(f)) <= TOL, (f, rel(sim.get_field(f), o.get(f)))
+        assert_parity(sim.get_field(f), o.get(f), f)
     for q in range(6):
-        assert rel(sim.get_psi(q), o.get(4 + q)) <= TOL, q
+        assert_parity(sim.get_psi(q), o.get(4 + q), ("psi", q))
     sim.destroy()
 
 
@@ -203,17 +216,21 @@ def test_degenerate_grids_parity(B, kernel, shape, cpml):
     sim.step(5)
     o.step(5)
     for f in range(4):
-        assert rel(sim.get_field(f), o.get(f)) <= TOL, (f, rel(sim.get_field(f), o.get(f)))
+        assert_parity(sim.get_field(f), o.get(f), f)
     for q in range(6):
-        assert rel(sim.get_psi(q), o.get(4 + q)) <= TOL, q
+        assert_parity(sim.get_psi(q), o.get(4 + q), ("psi", q))
     sim.destroy()
 
 
-@pytest.mark.parametrize("kernel", [1, 0])
-@pytest.mark.parametrize("shape,cpml", [((70, 45, 37), (5, 9, 0, 7, 6, 0)), ((124, 18, 21), (12, 12, 4, 4, 8, 8)), ((133, 18, 21), (0,) * 6)])
+@pytest.mark.parametrize("kernel", [1, 0, 2])
+@pytest.mark.parametrize("shape,cpml", [((70, 45, 37), (5, 9, 0, 7, 6, 0)), ((124, 18, 21), (12, 12, 4, 4, 8, 8)), ((133, 18, 21), (0,) * 6),
+                                        ((136, 40, 90), (12, 12, 8, 8, 10, 10))])
 def test_heterogeneous_density_parity(B, kernel, shape, cpml):
-    """SURVEY NEXT-3 (reading R6): rho(x) and c(x) both heterogeneous; dt/(rho_bar dx) at the half nodes."""
+    """SURVEY NEXT-3 (reading R6): rho(x) and c(x) both heterogeneous; dt/(rho_bar dx) at the half nodes.
+    All three kernel families, the single-pass step included (three more TMA tiles per stage)."""
     tot = tuple(shape[a] + cpml[2 * a] + cpml[2 * a + 1] for a in range(3))
+    if kernel == 2 and tot[0] % 4:
+        pytest.skip("FDTD_KERNEL_FUSED needs Nx % 4 == 0")
     rng = np.random.default_rng(3)
     c = (1.0 + 0.3 * rng.random(tot[::-1])).astype(np.float32)
     rho = (0.8 + 0.7 * rng.random(tot[::-1])).astype(np.float32)
@@ -232,14 +249,12 @@ def test_heterogeneous_density_parity(B, kernel, shape, cpml):
     sim.step(8)
     o.step(8)
     for f in range(4):
-        assert rel(sim.get_field(f), o.get(f)) <= TOL, (f, rel(sim.get_field(f), o.get(f)))
+        assert_parity(sim.get_field(f), o.get(f), f)
     for q in range(6):
-        assert rel(sim.get_psi(q), o.get(4 + q)) <= TOL, q
+        assert_parity(sim.get_psi(q), o.get(4 + q), ("psi", q))
     sim.set_model(c, np.full(tot[::-1], 2.0, np.float32))           # back to a uniform density: the scalar path again
     sim.step(1)
     sim.destroy()
-    with pytest.raises(B.FdtdError):                                # the single-pass step is not built for this
-        B.Fdtd((16,) * 3, dt=0.4, kernel=B.FDTD_KERNEL_FUSED, density=B.FDTD_DENSITY_ARRAY)
 
 
 def test_cpml_reflection_falls_with_thickness(B):
@@ -348,10 +363,10 @@ def test_sources_sharing_a_node_and_steps_before_set_sources(B, kernel):
     sim.step(steps - 4)
     o.step(steps - 4)
     for f in range(4):
-        assert rel(sim.get_field(f), o.get(f)) <= TOL, f
+        assert_parity(sim.get_field(f), o.get(f), f)
     sim.step(3)                                  # past the end of the table: nothing is injected, nothing breaks
     o.step(3)
-    assert rel(sim.get_field(0), o.get(0)) <= TOL
+    assert_parity(sim.get_field(0), o.get(0), "p after the table has ended")
     sim.destroy()
 
 
