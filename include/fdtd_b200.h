@@ -86,6 +86,11 @@ typedef struct {
   int32_t density;        /* FDTD_DENSITY_UNIFORM / FDTD_DENSITY_ARRAY                                       */
   int32_t medium;         /* FDTD_MEDIUM_ARRAY (default) / FDTD_MEDIUM_UNIFORM                               */
   int32_t precision;      /* FDTD_PRECISION_FP32 (default) / FDTD_PRECISION_FP64                             */
+  int32_t time_block;     /* k = 0 / 1: one time step per pass over the grid.  k >= 2 (FDTD_KERNEL_FUSED,    */
+                          /* monolithic): k steps per pass over z slabs, each slab recomputing a ghost of    */
+                          /* 2r = 8 planes per remaining step on both sides (the enlarged ghost of P:42,     */
+                          /* P:82 inside one GPU); two more copies of the state; same bits as k = 1          */
+  int32_t time_block_planes; /* slab thickness for time_block >= 2; 0 = sized to keep a slab's planes in L2  */
   int32_t device;         /* CUDA device ordinal                                                             */
   void* stream;           /* cudaStream_t the work is enqueued on (0 = legacy default stream)                */
   void* workspace;        /* DEVICE memory, 256-byte aligned, owned by the caller, must outlive the context  */
@@ -173,6 +178,11 @@ int fdtd_coeffs(float out_host[4]);
  * tiled ones do not apply (FDTD_PERIODIC, or a total Nx that is not a multiple of 4: they move whole float4s); this
  * call is how a caller finds out. */
 int fdtd_kernel_in_use(const fdtd_ctx* ctx);
+
+/* time_block >= 2: plane-steps computed (ghost planes included) and plane-steps owned since fdtd_create, into
+ * out_host[0], out_host[1]; their ratio is the redundant compute of the temporal blocking (P:315 reports the same trade
+ * across GPUs).  Zeros for a context without time blocking. */
+int fdtd_time_block_stats(const fdtd_ctx* ctx, int64_t out_host[2]);
 
 /* Number of kernel launches (the library's own kernels) enqueued since the context was created. */
 int64_t fdtd_launch_count(const fdtd_ctx* ctx);

@@ -25,7 +25,7 @@ FDTD_OK, FDTD_EINVAL, FDTD_EWORKSPACE, FDTD_ECUDA, FDTD_EUNSUPPORTED = 0, -1, -2
 EXPORTS = [
     "fdtd_workspace_bytes", "fdtd_create", "fdtd_set_model", "fdtd_set_sources", "fdtd_step", "fdtd_step_profiled", "fdtd_get_field",
     "fdtd_get_field_box", "fdtd_set_field", "fdtd_get_field_f64", "fdtd_set_field_f64", "fdtd_get_psi_f64", "fdtd_fill_hash", "fdtd_get_psi", "fdtd_field_absmax", "fdtd_cpml_table",
-    "fdtd_coeffs", "fdtd_kernel_in_use", "fdtd_launch_count", "fdtd_dims", "fdtd_destroy", "fdtd_last_error",
+    "fdtd_coeffs", "fdtd_time_block_stats", "fdtd_kernel_in_use", "fdtd_launch_count", "fdtd_dims", "fdtd_destroy", "fdtd_last_error",
 ]
 
 
@@ -48,6 +48,8 @@ class fdtd_params(C.Structure):
         ("density", C.c_int32),
         ("medium", C.c_int32),
         ("precision", C.c_int32),
+        ("time_block", C.c_int32),
+        ("time_block_planes", C.c_int32),
         ("device", C.c_int32),
         ("stream", C.c_void_p),
         ("workspace", C.c_void_p),
@@ -88,6 +90,7 @@ def _load():
     L.fdtd_launch_count.argtypes = [vp]
     L.fdtd_dims.argtypes = [vp, vp]
     L.fdtd_kernel_in_use.argtypes = [vp]
+    L.fdtd_time_block_stats.argtypes = [vp, vp]
     L.fdtd_destroy.argtypes = [vp]
     L.fdtd_last_error.restype = C.c_char_p
     return L
@@ -113,7 +116,7 @@ def fdtd_coeffs():
 
 def make_params(n_interior, cpml=(0,) * 6, dx=1.0, dt=0.4, cpml_order=2, cpml_R0=1e-5, cpml_kappa_max=1.0,
                 cpml_alpha_max=0.0, cpml_c_ref=1.0, boundary=FDTD_WALL, decomp=(1, 1, 1), ghost=0, substeps=0,
-                kernel=FDTD_KERNEL_AUTO, density=FDTD_DENSITY_UNIFORM, medium=FDTD_MEDIUM_ARRAY, precision=FDTD_PRECISION_FP32, device=0):
+                kernel=FDTD_KERNEL_AUTO, density=FDTD_DENSITY_UNIFORM, medium=FDTD_MEDIUM_ARRAY, precision=FDTD_PRECISION_FP32, time_block=0, time_block_planes=0, device=0):
     p = fdtd_params()
     p.n_interior[:] = [int(v) for v in n_interior]
     p.cpml[:] = [int(v) for v in cpml]
@@ -124,6 +127,7 @@ def make_params(n_interior, cpml=(0,) * 6, dx=1.0, dt=0.4, cpml_order=2, cpml_R0
     p.decomp[:] = [int(v) for v in decomp]
     p.ghost, p.substeps_per_exchange = int(ghost), int(substeps)
     p.kernel, p.density, p.medium, p.precision, p.device = int(kernel), int(density), int(medium), int(precision), int(device)
+    p.time_block, p.time_block_planes = int(time_block), int(time_block_planes)
     return p
 
 
@@ -242,6 +246,12 @@ class Fdtd:
         a, b, ik = (np.zeros(n, np.float32) for _ in range(3))
         _check(lib.fdtd_cpml_table(self._h, int(axis), int(half), a.ctypes.data, b.ctypes.data, ik.ctypes.data), "fdtd_cpml_table")
         return a, b, ik
+
+    def time_block_stats(self):
+        """-> (plane-steps computed, plane-steps owned) of the time-blocked mode."""
+        out = np.zeros(2, np.int64)
+        _check(lib.fdtd_time_block_stats(self._h, out.ctypes.data), "fdtd_time_block_stats")
+        return int(out[0]), int(out[1])
 
     def kernel_in_use(self):
         return int(lib.fdtd_kernel_in_use(self._h))

@@ -93,6 +93,8 @@ Geometry make_geometry(const fdtd_params& P) {
   if (P.density != FDTD_DENSITY_UNIFORM && P.density != FDTD_DENSITY_ARRAY) return bad("unknown density selector");
   if (P.medium != FDTD_MEDIUM_ARRAY && P.medium != FDTD_MEDIUM_UNIFORM) return bad("unknown medium selector");
   if (P.precision != FDTD_PRECISION_FP32 && P.precision != FDTD_PRECISION_FP64) return bad("unknown precision selector");
+  if (P.time_block < 0 || P.time_block > 8 || P.time_block_planes < 0) return bad("time_block must be 0 .. 8 and time_block_planes >= 0");
+  if (P.time_block > 1 && P.kernel != FDTD_KERNEL_FUSED) return bad("time_block needs FDTD_KERNEL_FUSED");
   if (P.precision == FDTD_PRECISION_FP64 && P.kernel == FDTD_KERNEL_FUSED)
     return bad("the fp64 verification precision runs the one-thread-per-point kernels only (FDTD_KERNEL_AUTO or FDTD_KERNEL_REF)");
   if (P.boundary == FDTD_PERIODIC)
@@ -102,6 +104,7 @@ Geometry make_geometry(const fdtd_params& P) {
       return bad("bad CPML parameters");
   const bool sub = G.nd[0] * G.nd[1] * G.nd[2] > 1;
   if (sub && P.precision == FDTD_PRECISION_FP64) return bad("the fp64 verification precision is monolithic only");
+  if (sub && P.time_block > 1) return bad("time_block is monolithic only");
   G.ghost = sub ? P.ghost : 0;
   G.msub = sub ? P.substeps_per_exchange : 0;
   if (sub) {
@@ -144,6 +147,11 @@ struct Domain {
   Sched sched;
   Sched sched_f;               // work decomposition of step_fused
   int fused_parity = 0;
+  // time_block >= 2: scratch states and the launch list of one block of k steps (slab by slab, step by step)
+  OutSet xs[2];
+  TMaps tm_xs[2];
+  struct TbLaunch { int zlo, zhi, in_state, out_state, step; const int4* table; int nitems; };   // states: 0 current, 1 out, 2 X, 3 Y
+  std::vector<TbLaunch> tb;
   long long* src_offset = nullptr;   // device, per source
 };
 
@@ -156,6 +164,9 @@ struct Layout {
     uint64_t f2[4], psi2[2][3][2];   // fused mode: second state
     uint64_t bq[3];                  // FDTD_DENSITY_ARRAY: dt/(rho_bar dx) at the half nodes of vx, vy, vz
     uint64_t items, items_cap;       // fused mode: item table of step_fused (int4 per item)
+    uint64_t fx[2][4], psix[2][2][3][2];   // time_block >= 2: scratch states X, Y (intermediate steps of a z slab)
+    uint64_t tb_items, tb_items_cap;       // ... and the item tables of its per-slab launches
+    int tb_planes;                         // ... slab thickness
   };
   std::vector<Dom> doms;
   uint64_t tab[2][3][3];
@@ -214,6 +225,29 @@ Layout make_layout(const fdtd_params& P, const Geometry& G) {
             d.psi2[fam][2][s] = take((uint64_t)d.pitch * d.n[1] * d.ln[2][s] * 4 + 16);
           }
       }
+      if (P.kernel == FDTD_KERNEL_FUSED && P.time_block > 1) {
+        for (int x = 0; x < (P.time_block > 2 ? 2 : 1); ++x) {
+          for (int f = 0; f < 4; ++f) d.fx[x][f] = take(vol);
+          for (int fam = 0; fam < 2; ++fam)
+            for (int s = 0; s < 2; ++s) {
+              d.psix[x][fam][0][s] = take((uint64_t)d.ln[0][s] * d.n[1] * d.n[2] * 4 + 16);
+              d.psix[x][fam][1][s] = take((uint64_t)d.pitch * d.ln[1][s] * d.n[2] * 4 + 16);
+              d.psix[x][fam][2][s] = take((uint64_t)d.pitch * d.n[1] * d.ln[2][s] * 4 + 16);
+            }
+        }
+        // slab thickness: given, or such that the planes one slab touches (fields in + out, all its steps) stay near 64 MB
+        // of the 126 MB L2; never thinner than the 8 planes of ghost one extra step costs on each side
+        int zs = P.time_block_planes;
+        if (zs <= 0) {
+          const double per_plane = (double)d.pitch * d.n[1] * 4 * 8;
+          zs = (int)(64e6 / per_plane) - 16 * (P.time_block - 1);
+        }
+        d.tb_planes = std::max(8, std::min(zs, d.n[2]));
+        const uint64_t tiles = (uint64_t)((d.n[0] + TX - 1) / TX) * ((d.n[1] + TY - 1) / TY);
+        const uint64_t nslab = (d.n[2] + d.tb_planes - 1) / d.tb_planes;
+        d.tb_items_cap = tiles * nslab * P.time_block * (1 + (d.tb_planes + 16 * P.time_block) / 64) + 16;
+        d.tb_items = take(d.tb_items_cap * 16);
+      }
       if (P.density == FDTD_DENSITY_ARRAY)
         for (int a = 0; a < 3; ++a) d.bq[a] = take(vol);
       d.src_off = take(MAX_SRC * sizeof(long long));
@@ -256,6 +290,8 @@ struct fdtd_ctx {
   float* d_wav;
   int64_t launches = 0;
   int64_t substeps_done = 0;    // sub-updates since the last halo exchange (subdomain mode)
+  int time_block = 1;           // steps advanced per z-slab pass (FDTD_KERNEL_FUSED)
+  int64_t plane_steps_computed = 0, plane_steps_owned = 0;   // time_block: redundant-compute counters (planes x steps)
   int grid_v = 0, grid_p = 0;       // resident CTAs of the whole GPU for each tiled kernel
 };
 
@@ -357,6 +393,73 @@ int launch_fused(fdtd_ctx* c, Domain& d) {
   return FDTD_OK;
 }
 
+// Items of step_fused for the planes [zlo, zhi) only (one z slab of the time-blocked mode): chunks of at most 64 planes,
+// slab-touching tiles first.
+void plan_items_range(const Domain& d, int zlo, int zhi, std::vector<int4>& table) {
+  const DomainView& v = d.v;
+  const int ntx = (v.nx + TX - 1) / TX, nty = (v.ny + TY - 1) / TY;
+  const int nch = std::max(1, (zhi - zlo + 63) / 64);
+  auto touches_slab = [&](int axis, int lo, int hi) {
+    return (v.ln[axis][0] > 0 && lo < v.ls[axis][0] + v.ln[axis][0] && hi > v.ls[axis][0]) ||
+           (v.ln[axis][1] > 0 && lo < v.ls[axis][1] + v.ln[axis][1] && hi > v.ls[axis][1]);
+  };
+  std::vector<int4> rest;
+  for (int c = 0; c < nch; ++c) {
+    const int z0 = zlo + (int)((long long)(zhi - zlo) * c / nch), z1 = zlo + (int)((long long)(zhi - zlo) * (c + 1) / nch);
+    for (int ty = 0; ty < nty; ++ty)
+      for (int tx = 0; tx < ntx; ++tx) {
+        const int x0 = tx * TX, y0 = ty * TY;
+        (touches_slab(0, x0, x0 + TX) || touches_slab(1, y0, y0 + TY) ? table : rest).push_back(make_int4(x0, y0, z0, z1));
+      }
+  }
+  table.insert(table.end(), rest.begin(), rest.end());
+}
+
+int launch_inject_range(fdtd_ctx* c, Domain& d, float* p, long long n, int zlo, int zhi);
+
+// k time steps in one pass over the z slabs (the single-device form of the paper's enlarged ghost, P:42, P:82,
+// blocked along z): for every slab [a, b) step j = 1..k is computed on [a - 8(k-j), b + 8(k-j)) — a ghost of 2r = 8 planes
+// per remaining step on each side, recomputed by the neighbouring slabs as well — so that the slab's planes can stay in L2
+// between its k launches.  Intermediate steps live in the scratch states X / Y, the last one goes to the out state, which
+// then becomes the current state.  Same arithmetic per point as k single steps: same bits.
+int do_time_block(fdtd_ctx* c) {
+  Domain& d = c->doms[0];
+  for (const auto& L : d.tb) {
+    DomainView vin = d.v;
+    const TMaps* tm = &d.tm;
+    if (L.in_state >= 2) {
+      const OutSet& I = d.xs[L.in_state - 2];
+      for (int f = 0; f < 4; ++f) vin.f[f] = I.f[f];
+      for (int fam = 0; fam < 2; ++fam)
+        for (int a = 0; a < 3; ++a)
+          for (int s = 0; s < 2; ++s) vin.psi[fam][a][s] = I.psi[fam][a][s];
+      tm = &d.tm_xs[L.in_state - 2];
+    }
+    const OutSet& O = L.out_state == 1 ? d.alt : d.xs[L.out_state - 2];
+    Sched S = d.sched_f;
+    S.table = L.table;
+    S.nitems = L.nitems;
+    S.counter = d.counters + 2 + d.fused_parity;
+    S.other = d.counters + 2 + (1 - d.fused_parity);
+    if (vin.bq[0]) step_fused<true><<<std::min(c->grid_f, S.nitems), FNT, f_smem_bytes<true>(), c->stream>>>(*tm, vin, O, S);
+    else step_fused<false><<<std::min(c->grid_f, S.nitems), FNT, f_smem_bytes<false>(), c->stream>>>(*tm, vin, O, S);
+    c->launches++;
+    CK(cudaGetLastError());
+    d.fused_parity ^= 1;
+    c->plane_steps_computed += L.zhi - L.zlo;
+    int r = launch_inject_range(c, d, O.f[0], c->step_index + L.step, L.zlo, L.zhi);
+    if (r) return r;
+  }
+  c->plane_steps_owned += (int64_t)d.v.nz * c->time_block;
+  c->step_index += c->time_block;
+  for (int f = 0; f < 4; ++f) std::swap(d.v.f[f], d.alt.f[f]);
+  for (int fam = 0; fam < 2; ++fam)
+    for (int a = 0; a < 3; ++a)
+      for (int s = 0; s < 2; ++s) std::swap(d.v.psi[fam][a][s], d.alt.psi[fam][a][s]);
+  std::swap(d.tm, d.tm_alt);
+  return FDTD_OK;
+}
+
 int launch_substep(fdtd_ctx* c, Domain& d, int which /*0 = v, 1 = p*/) {
   const DomainView& v = d.v;
   if (c->use_ref) {
@@ -387,14 +490,24 @@ int launch_inject(fdtd_ctx* c) {
   if (c->nsrc == 0 || n >= c->wlen) return FDTD_OK;
   for (size_t k = 0; k < c->doms.size(); ++k) {
     if (c->fp64) {
-      SourceViewT<double> S{c->nsrc, c->wlen, c->doms[k].src_offset, c->doms[k].v64.f[0], c->d_wav};
+      SourceViewT<double> S{c->nsrc, c->wlen, c->doms[k].src_offset, c->doms[k].v64.f[0], c->d_wav, 0, 0x7fffffffffffffffLL};
       inject_sources<<<1, 64, 0, c->stream>>>(S, n);
     } else {
-      SourceView S{c->nsrc, c->wlen, c->doms[k].src_offset, c->doms[k].v.f[0], c->d_wav};
+      SourceView S{c->nsrc, c->wlen, c->doms[k].src_offset, c->doms[k].v.f[0], c->d_wav, 0, 0x7fffffffffffffffLL};
       inject_sources<<<1, 64, 0, c->stream>>>(S, n);
     }
     c->launches++;
   }
+  CK(cudaGetLastError());
+  return FDTD_OK;
+}
+
+// the sources whose plane lies in [zlo, zhi) into the pressure array p of a state that is not the current one (time_block)
+int launch_inject_range(fdtd_ctx* c, Domain& d, float* p, long long n, int zlo, int zhi) {
+  if (c->nsrc == 0 || n >= c->wlen) return FDTD_OK;
+  SourceView S{c->nsrc, c->wlen, d.src_offset, p, c->d_wav, (long long)zlo * d.v.plane, (long long)zhi * d.v.plane};
+  inject_sources<<<1, 64, 0, c->stream>>>(S, n);
+  c->launches++;
   CK(cudaGetLastError());
   return FDTD_OK;
 }
@@ -758,6 +871,13 @@ fdtd_ctx* fdtd_create(const fdtd_params* P) {
             for (int a = 0; a < 3; ++a)
               for (int s = 0; s < 2; ++s) d.alt.psi[fam][a][s] = (float*)(c->ws + ld.psi2[fam][a][s]);
           bad = make_maps(d.tm_alt, d.alt.f);
+          for (int x = 0; x < (P->time_block > 2 ? 2 : (P->time_block > 1 ? 1 : 0)) && !bad; ++x) {
+            for (int f = 0; f < 4; ++f) d.xs[x].f[f] = (float*)(c->ws + ld.fx[x][f]);
+            for (int fam = 0; fam < 2; ++fam)
+              for (int a = 0; a < 3; ++a)
+                for (int s = 0; s < 2; ++s) d.xs[x].psi[fam][a][s] = (float*)(c->ws + ld.psix[x][fam][a][s]);
+            bad = make_maps(d.tm_xs[x], d.xs[x].f);
+          }
         }
         if (bad) { delete c; return nullptr; }
       }
@@ -790,6 +910,36 @@ fdtd_ctx* fdtd_create(const fdtd_params* P) {
             (e = cudaStreamSynchronize(c->stream)) != cudaSuccess)
           return fail(c, e, "cudaMemcpyAsync(item table)");
         d.sched_f.table = (const int4*)(c->ws + L.doms[k].items);
+      }
+      c->time_block = std::max(1, (int)P->time_block);
+      if (c->time_block > 1) {
+        Domain& d = c->doms[0];
+        const Layout::Dom& ld = L.doms[0];
+        const int k = c->time_block, nz = d.v.nz, zs = ld.tb_planes;
+        std::vector<int4> all;
+        std::vector<size_t> first;
+        for (int a = 0; a < nz; a += zs) {
+          const int b = std::min(nz, a + zs);
+          for (int j = 1; j <= k; ++j) {
+            const int ext = 8 * (k - j);
+            Domain::TbLaunch T{};
+            T.zlo = std::max(0, a - ext); T.zhi = std::min(nz, b + ext);
+            T.in_state = j == 1 ? 0 : 2 + (j - 2) % 2;
+            T.out_state = j == k ? 1 : 2 + (j - 1) % 2;
+            T.step = j - 1;
+            std::vector<int4> t;
+            plan_items_range(d, T.zlo, T.zhi, t);
+            T.nitems = (int)t.size();
+            first.push_back(all.size());
+            all.insert(all.end(), t.begin(), t.end());
+            d.tb.push_back(T);
+          }
+        }
+        if (all.size() > ld.tb_items_cap) { set_err("time-block item tables larger than their workspace slot"); delete c; return nullptr; }
+        if ((e = cudaMemcpyAsync(c->ws + ld.tb_items, all.data(), all.size() * sizeof(int4), cudaMemcpyHostToDevice, c->stream)) != cudaSuccess ||
+            (e = cudaStreamSynchronize(c->stream)) != cudaSuccess)
+          return fail(c, e, "cudaMemcpyAsync(time-block item tables)");
+        for (size_t t = 0; t < d.tb.size(); ++t) d.tb[t].table = (const int4*)(c->ws + ld.tb_items) + first[t];
       }
     }
   }
@@ -929,6 +1079,11 @@ int fdtd_step(fdtd_ctx* c, int32_t n) {
   if (!c || n < 0) return FDTD_EINVAL;
   for (int s = 0; s < n; ++s) {
     int r;
+    if (c->time_block > 1 && n - s >= c->time_block) {      // k steps per pass over the z slabs, sources included
+      if ((r = do_time_block(c))) return r;
+      s += c->time_block - 1;
+      continue;
+    }
     if (c->fused) {
       if ((r = do_fused_step(c))) return r;   // both sub-updates in one pass (a7)
     } else {
@@ -945,7 +1100,7 @@ int fdtd_step_profiled(fdtd_ctx* c, int32_t n, double out_ms[4]) {
   // One CUDA event on the launching stream after every launch group; the interval that ends at a mark is
   // charged to the mark's category (0 = update_v / step_fused, 1 = update_p, 2 = inject, 3 = exchange).  The events are
   // created up front and destroyed on every way out.
-  std::vector<cudaEvent_t> ev((size_t)n * 5 + 1, nullptr);
+  std::vector<cudaEvent_t> ev((size_t)n * 5 + 2, nullptr);
   std::vector<int> cat(ev.size(), -1);
   size_t used = 0;
   int r = FDTD_OK;
@@ -958,6 +1113,12 @@ int fdtd_step_profiled(fdtd_ctx* c, int32_t n, double out_ms[4]) {
   };
   if (ce == cudaSuccess) mark(-1);
   for (int s = 0; s < n && !r && ce == cudaSuccess; ++s) {
+    if (c->time_block > 1 && n - s >= c->time_block) {
+      r = do_time_block(c);
+      mark(0);
+      s += c->time_block - 1;
+      continue;
+    }
     if (c->fused) {
       if (c->doms.size() > 1 && c->substeps_done % c->G.msub == 0) {
         r = exchange_halos(c);
@@ -990,6 +1151,12 @@ int fdtd_step_profiled(fdtd_ctx* c, int32_t n, double out_ms[4]) {
     if (e) cudaEventDestroy(e);
   CK(ce);
   return r;
+}
+
+int fdtd_time_block_stats(const fdtd_ctx* c, int64_t out[2]) {
+  if (!c || !out) return FDTD_EINVAL;
+  out[0] = c->plane_steps_computed; out[1] = c->plane_steps_owned;
+  return FDTD_OK;
 }
 
 int fdtd_kernel_in_use(const fdtd_ctx* c) {

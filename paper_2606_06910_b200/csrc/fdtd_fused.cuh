@@ -8,7 +8,7 @@
 // a ghost of 2r = 8 cells per full step, exactly the paper's count.  Inside one GPU that ghost is
 //   x, y : recomputed.  A 64x16 tile computes vx_new on 72x16 and vy_new on 64x23 points; the extra strips are done
 //          by four "halo" warps, the tile itself by eight "main" warps, and the values meet in a double-buffered
-//          shared-memory exchange (E) guarded by one mbarrier per buffer;
+//          shared-memory exchange (E, three buffers) guarded by one mbarrier per buffer;
 //   z    : streamed.  Each main thread keeps p_old[k..k+7] and vz_new[k-4..k+3] of its four x-points in registers.
 // Because neighbouring tiles re-read old values that the owner is about to overwrite, the step is out of place:
 // state "in" -> state "out" (fields and psi), swapped by the host after every launch.
@@ -55,7 +55,8 @@ constexpr int F_OFF_BZ = F_OFF_BY + F_VY_FLOATS;
 template <bool HB> __host__ __device__ constexpr int f_stage_floats() { return HB ? F_OFF_BZ + TILE_FLOATS : F_OFF_BX; }
 constexpr int E_OFF_VY = F_VX_FLOATS;            // exchange buffer: [vx_new 16 x 72 | vy_new 24 x 64]
 constexpr int E_FLOATS = F_VX_FLOATS + TX * EVY_ROWS;
-template <bool HB> __host__ __device__ constexpr int f_smem_bytes() { return (FNS * f_stage_floats<HB>() + 2 * E_FLOATS) * 4; }
+constexpr int E_BUFS = 3;                        // three exchange buffers: the halo warps may run two planes ahead of the main warps
+template <bool HB> __host__ __device__ constexpr int f_smem_bytes() { return (FNS * f_stage_floats<HB>() + E_BUFS * E_FLOATS) * 4; }
 static_assert((F_PB_FLOATS * 4) % 128 == 0 && (F_VX_FLOATS * 4) % 128 == 0 && (F_VY_FLOATS * 4) % 128 == 0 && (E_FLOATS * 4) % 128 == 0,
               "TMA destinations must stay 128-B aligned");
 static_assert(f_smem_bytes<true>() <= 227 * 1024 - 4096, "stage ring + exchange buffers + static shared memory must fit one SM");
@@ -91,7 +92,7 @@ __device__ __forceinline__ void fill_tab_cache(const DomainView& D, TabCache& T,
 struct FusedBars {
   uint64_t* full;     // [FNS] TMA stage landed
   uint64_t* empty;    // [FNS] every warp has read the stage
-  uint64_t* efull;    // [2]   every warp has written its part of the exchange buffer
+  uint64_t* efull;    // [E_BUFS] every warp has written its part of the exchange buffer
 };
 
 __device__ __forceinline__ void warp_arrive(uint64_t* bar) {
@@ -239,9 +240,9 @@ __device__ __forceinline__ void fused_plane(const DomainView& D, const OutSet& O
     vy4 = upd4(vy4, K.By, K.By, K.By, dyv);
   }
   if (K.active) { st4(O.f[1] + C.goff, vx4); st4(O.f[2] + C.goff, vy4); }
-  const unsigned eb = C.eit & 1;
+  const unsigned eb = C.eit % E_BUFS;
   float* E = ebuf + eb * E_FLOATS;
-  // every main warp has passed the efull wait of the previous plane, so nobody still reads this buffer (see step_fused)
+  // this buffer was last read for plane eit-3, and every main warp is at most one plane away from this one
   st4(E + K.exo, vx4);
   st4(E + E_OFF_VY + 4 * TX + K.toff, vy4);
   warp_arrive(&Q.efull[eb]);
@@ -261,7 +262,7 @@ __device__ __forceinline__ void fused_plane(const DomainView& D, const OutSet& O
 
   // ---- pressure sub-update at plane k
   C.pre = mbar_test(&Q.full[(C.it + 1) % FNS], ((C.it + 1) / FNS) & 1);      // probe the next stage now, use the answer next iteration
-  mbar_wait(&Q.efull[eb], (C.eit >> 1) & 1);
+  mbar_wait(&Q.efull[eb], (C.eit / E_BUFS) & 1);
   const float* xr = E + K.exo;
   V4 dxp = diff_x<false>(ld4(xr - 4), vx4, ld4(xr + 4));
   const float* col = E + E_OFF_VY + K.toff;                       // row ty of E.vy <-> y = j-4
@@ -482,11 +483,12 @@ __device__ __forceinline__ void fused_halo(const DomainView& D, float* smem, flo
           vx4 = upd4(vx4, Bvx, Bvx, Bx3, dxv);
         }
       }
-      const unsigned eb = eit & 1;
+      const unsigned eb = eit % E_BUFS;
       float* E = ebuf + eb * E_FLOATS;
-      // this buffer was last read for plane eit-2; every main warp is past that once the previous plane's efull phase
-      // is complete (a main warp arrives there only after it has finished reading the plane before)
-      if (eit > 0) mbar_wait(&Q.efull[eb ^ 1], ((eit - 1) >> 1) & 1);
+      // this buffer was last read for plane eit-3; every main warp is past that once the efull phase of plane eit-2 is
+      // complete (a main warp arrives there only after it has finished reading the plane before), so the halo warps can
+      // run up to two planes ahead and their psi / stage latencies stay off the main warps' critical path
+      if (eit > 1) mbar_wait(&Q.efull[(eit - 2) % E_BUFS], ((eit - 2) / E_BUFS) & 1);
       st4(E + E_OFF_VY + eyo, vy4);
       if (do_x) st4(E + exo, vx4);
       warp_arrive(&Q.efull[eb]);
@@ -501,14 +503,15 @@ __global__ void __launch_bounds__(FNT, 1) step_fused(const __grid_constant__ TMa
   extern __shared__ __align__(128) unsigned char smem_raw[];
   float* smem = reinterpret_cast<float*>(smem_raw);
   float* ebuf = smem + FNS * f_stage_floats<HB>();
-  __shared__ __align__(8) uint64_t bars[2 * FNS + 2];
+  __shared__ __align__(8) uint64_t bars[2 * FNS + E_BUFS];
   __shared__ int s_item;
   __shared__ __align__(16) TabCache tabc;
   const FusedBars Q{bars, bars + FNS, bars + 2 * FNS};
   if (threadIdx.x == 0) {
 #pragma unroll
     for (int s = 0; s < FNS; ++s) { mbar_init(&Q.full[s], 1); mbar_init(&Q.empty[s], FNW); }
-    mbar_init(&Q.efull[0], FNW); mbar_init(&Q.efull[1], FNW);
+#pragma unroll
+    for (int b = 0; b < E_BUFS; ++b) mbar_init(&Q.efull[b], FNW);
     fence_barrier_init();
     if (blockIdx.x == 0) *S.other = 0u;
   }

@@ -694,6 +694,7 @@ struct SourceViewT {
   const long long* offset;   // flat element offset of each source in its domain's p array, or -1 if not held
   T* p;
   const float* wav;
+  long long lo, hi;          // only sources whose offset lies in [lo, hi) (a plane range; everything: 0, LLONG_MAX)
 };
 typedef SourceViewT<float> SourceView;
 template <class T>
@@ -701,7 +702,7 @@ __global__ void inject_sources(SourceViewT<T> S, long long n) {
   if (n >= S.len) return;
   for (int s = threadIdx.x; s < S.n; s += blockDim.x) {
     const long long off = S.offset[s];
-    if (off < 0) continue;
+    if (off < S.lo || off >= S.hi) continue;              // not held by this domain (-1), or outside the plane range
     bool first = true;
     for (int t = 0; t < s; ++t) first = first && S.offset[t] != off;
     if (!first) continue;

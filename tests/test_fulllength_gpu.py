@@ -105,7 +105,7 @@ def test_config3_full_length_1000_steps(B):
       * all 1000 steps against the oracle with its FTZ/DAZ switch on (run in a process of its own, see
         tests/oracle_config3_ftz.py): flushing the denormals of the pulse's leading edge gives another, equally valid
         fp32 realisation of the run, so this one is held to BASELINE's tolerance — 1e-4 of max|oracle| per field; the six
-        memory variables, which R17 reports informally, to 2e-4 (two realisations within 1e-4 of the exact recurrence)."""
+        memory variables included (measured: p 9e-7, v 1.1e-5, psi 7.2e-5)."""
     import os
     import subprocess
     import sys
@@ -142,7 +142,7 @@ def test_config3_full_length_1000_steps(B):
                 elif k == 2:
                     e, s = _rel(got[k][2][i - 4], r)
                     print("config3 x1000 kernel 2 psi %d vs the FTZ oracle: max rel err %.3e" % (i - 4, e))
-                    assert s > 0 and e <= 2 * TOL, (i, e)
+                    assert s > 0 and e <= TOL, (i, e)
             del r
     # the IEEE oracle over the first PREFIX3 steps: bit for bit
     o = Oracle(w.n_interior, w.cpml, **w.cpml_kwargs())
