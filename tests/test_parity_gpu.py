@@ -260,7 +260,7 @@ def test_heterogeneous_density_parity(B, kernel, shape, cpml):
 def test_cpml_reflection_falls_with_thickness(B):
     """P:170, Table 8 (trend only; the paper's procedure is unstated): against a reference run in a box so large
     that nothing returns, a CPML-bounded run differs by orders of magnitude less than a wall-bounded one, and a thicker
-    layer reflects less.  Small version of paper_2606_06910_b200.reflection_study (kappa = 1 sets)."""
+    layer reflects less.  Small version of paper_2606_06910_b200.reflection_study."""
     from paper_2606_06910_b200 import reflection_study as rs
 
     interior, steps = 48, 200
@@ -276,6 +276,19 @@ def test_cpml_reflection_falls_with_thickness(B):
         ratio[L] = max(float(np.abs(a - b).max()) for a, b in zip(t, ref)) / incident
     assert ratio[0] > 0.5                                   # walls send the pulse back
     assert ratio[8] < 5e-3 and ratio[16] < ratio[8] / 3     # the layer absorbs it; a thicker one absorbs more
+    # The paper's own set (q = 3, R = 1e-8, alpha_max = 0.05 sigma_max; Table 2): with kappa_max = 1 it shows the same fall;
+    # with Table 2's kappa_max = 5 the layer still absorbs (two orders below a wall) but the ratio stays on a plateau that
+    # does not fall with thickness and lies above the kappa_max = 1 value (profiles/r02_studies.md, DESIGN.md NEXT-2).
+    paper = {}
+    for kmax in (1.0, 5.0):
+        for L in (8, 16):
+            smax = -4.0 * math.log(1e-8) / (2.0 * L)
+            pk = dict(cpml_order=3, cpml_R0=1e-8, cpml_kappa_max=kmax, cpml_alpha_max=0.05 * smax)
+            t = rs.run(interior, L, steps, 20, 20, 0, pk, B.FDTD_KERNEL_FUSED)
+            paper[kmax, L] = max(float(np.abs(a - b).max()) for a, b in zip(t, ref)) / incident
+    assert paper[1.0, 8] < 5e-3 and paper[1.0, 16] < paper[1.0, 8] / 3
+    assert paper[5.0, 8] < 2e-2 and paper[5.0, 16] < 2e-2
+    assert paper[5.0, 16] > 3 * paper[1.0, 16]
 
 
 def test_periodic_dispersion_on_gpu(B):
