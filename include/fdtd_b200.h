@@ -32,8 +32,8 @@ enum {
   FDTD_EINVAL = -1,     /* bad size / parameter (dt <= 0, grid smaller than the layers, source out of range ...) */
   FDTD_EWORKSPACE = -2, /* workspace NULL, misaligned (256 B) or smaller than fdtd_workspace_bytes() */
   FDTD_ECUDA = -3,      /* a CUDA runtime / driver call failed; fdtd_last_error() has the text */
-  FDTD_EUNSUPPORTED = -4 /* valid per the paper but not built in this configuration (e.g. a density array with   */
-                         /* FDTD_KERNEL_FUSED, or without params.density = FDTD_DENSITY_ARRAY)                   */
+  FDTD_EUNSUPPORTED = -4 /* valid per the paper but not built in this configuration (e.g. a density array without */
+                         /* params.density = FDTD_DENSITY_ARRAY, or FDTD_PRECISION_FP64 with FDTD_KERNEL_FUSED)   */
 };
 
 enum { FDTD_P = 0, FDTD_VX = 1, FDTD_VY = 2, FDTD_VZ = 3 };                 /* field selectors */
