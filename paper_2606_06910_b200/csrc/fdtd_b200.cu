@@ -333,7 +333,7 @@ void plan_items(Domain& d, int grid) {
   S.nitems = (int)(tiles * S.nzc);
 }
 
-// step_fused items: the z lead-in of an item is 14 planes (7 of them load only a p tile), so chunks are long.
+// step_fused items: every item pays a lead-in of 14 planes (batched into 3 - 4 pipeline stages), so chunks are long.
 // Items are handed out from a table, most expensive first (a tile x z-chunk that touches an x / y slab costs about 1.5x
 // an interior one per plane), with z-chunks that shrink from round to round, so that the CTAs finish together; within one
 // cost class the order stays x-fastest, so that concurrently running items are neighbours and share their halos in L2.

@@ -37,7 +37,15 @@ constexpr int FNW = FW_MAIN + FW_HALO;           // 12 consumer warps
 constexpr int FNT = (FNW + FW_PROD) * 32;        // 512 threads = 4 warps per SM sub-partition
 constexpr int F_REGS_MAIN = 200, F_REGS_HALO = 80, F_REGS_PROD = 32;   // 2 x 200 + 80 + 32 = 512 registers per sub-partition lane
 constexpr int FNS = 4;                           // TMA ring stages
-constexpr int F_LEAD = 14;                       // ring iterations of an item before its first output plane
+// Lead-in of an item (tile x z-chunk): before the first output plane z0 the rings need p_old[z0-7 .. z0+6] and
+// vz_new[z0-4 .. z0+2].  A lead-in plane carries one or two 4-KB tiles, far less than a stage holds, and with one plane per
+// stage the lead-in ran at the latency of four TMA round trips per four planes (980 cycles per plane, measured).  So the
+// lead-in planes are batched: stage 0 of an item holds the seven p tiles of planes z0-7 .. z0-1, the next L2S stages hold L2P
+// planes each of (p tile of plane m, vz tile of plane m-4 [, dt/(rho_bar dx) of vz]) for m = z0 .. z0+6.
+template <bool HB> __host__ __device__ constexpr int f_lead2_planes() { return HB ? 3 : 4; }      // planes per lead-in-2 stage
+template <bool HB> __host__ __device__ constexpr int f_lead2_stages() { return HB ? 3 : 2; }      // 3+3+1 or 4+3 planes
+template <bool HB> __host__ __device__ constexpr int f_lead2_tiles() { return HB ? 3 : 2; }       // tiles per lead-in-2 plane
+template <bool HB> __host__ __device__ constexpr int f_lead() { return 1 + f_lead2_stages<HB>(); } // stages before the first output plane
 constexpr int BW = TX + 16;                      // p box: columns x0-8 .. x0+TX+7
 constexpr int BH = TY + 14;                      // p box: rows    y0-7 .. y0+TY+6
 constexpr int EVY_ROWS = TY + 8;                 // vy_new exchange rows y0-4 .. y0+TY+3 (the last one is never read)
@@ -52,7 +60,10 @@ constexpr int F_OFF_KC = F_OFF_VY + F_VY_FLOATS;
 constexpr int F_OFF_BX = F_OFF_KC + TILE_FLOATS; // HB only
 constexpr int F_OFF_BY = F_OFF_BX + F_VX_FLOATS;
 constexpr int F_OFF_BZ = F_OFF_BY + F_VY_FLOATS;
-template <bool HB> __host__ __device__ constexpr int f_stage_floats() { return HB ? F_OFF_BZ + TILE_FLOATS : F_OFF_BX; }
+template <bool HB> __host__ __device__ constexpr int f_stage_floats() {
+  return HB ? F_OFF_BZ + TILE_FLOATS : (F_OFF_BX > 8 * TILE_FLOATS ? F_OFF_BX : 8 * TILE_FLOATS);   // a lead-in-2 stage holds 4 x 2 tiles
+}
+static_assert(7 * TILE_FLOATS <= f_stage_floats<false>() && 9 * TILE_FLOATS <= f_stage_floats<true>(), "lead-in batches must fit a stage");
 constexpr int E_OFF_VY = F_VX_FLOATS;            // exchange buffer: [vx_new 16 x 72 | vy_new 24 x 64]
 constexpr int E_FLOATS = F_VX_FLOATS + TX * EVY_ROWS;
 constexpr int E_BUFS = 3;                        // three exchange buffers: the halo warps may run two planes ahead of the main warps
@@ -100,29 +111,41 @@ __device__ __forceinline__ void warp_arrive(uint64_t* bar) {
   if ((threadIdx.x & 31) == 0) mbar_arrive(bar);
 }
 
+// Stage s of an item: s = 0 and 1 .. L2S are the batched lead-in stages, s >= f_lead() carries output plane k = z0 + s - f_lead().
 template <bool HB>
-__device__ __forceinline__ void fused_issue(const TMaps& tm, float* smem, uint64_t* full, unsigned slot, int m, int x0, int y0, int z0,
+__device__ __forceinline__ void fused_issue(const TMaps& tm, float* smem, uint64_t* full, unsigned slot, int s, int x0, int y0, int z0,
                                             bool has_kc) {
-  const int k = m - 7;
-  const bool vz = m >= z0, out = k >= z0;
+  constexpr int L2P = f_lead2_planes<HB>(), L2S = f_lead2_stages<HB>(), TPP = f_lead2_tiles<HB>();
   uint64_t* bar = &full[slot];
   float* st = smem + slot * f_stage_floats<HB>();
-  mbar_expect_tx(bar, TILE_BYTES + (vz ? (HB ? 2 : 1) * TILE_BYTES : 0) +
-                          (out ? (F_PB_FLOATS + (HB ? 2 : 1) * (F_VX_FLOATS + F_VY_FLOATS)) * 4 + (has_kc ? TILE_BYTES : 0) : 0));
-  tma_load_3d(st + F_OFF_PT, &tm.tile[0], bar, x0, y0, m);
-  if (vz) {
-    tma_load_3d(st + F_OFF_VZ, &tm.tile[3], bar, x0, y0, m - 4);
-    if (HB) tma_load_3d(st + F_OFF_BZ, &tm.bq_tile, bar, x0, y0, m - 4);
+  if (s == 0) {
+    mbar_expect_tx(bar, 7 * TILE_BYTES);
+#pragma unroll
+    for (int j = 0; j < 7; ++j) tma_load_3d(st + j * TILE_FLOATS, &tm.tile[0], bar, x0, y0, z0 - 7 + j);
+    return;
   }
-  if (out) {
-    tma_load_3d(st, &tm.p_box, bar, x0 - 8, y0 - 7, k);
-    tma_load_3d(st + F_OFF_VX, &tm.vx_halo, bar, x0 - 4, y0, k);
-    tma_load_3d(st + F_OFF_VY, &tm.vy_halo, bar, x0, y0 - 4, k);
-    if (has_kc) tma_load_3d(st + F_OFF_KC, &tm.tile[4], bar, x0, y0, k);
-    if (HB) {
-      tma_load_3d(st + F_OFF_BX, &tm.bq_halo[0], bar, x0 - 4, y0, k);
-      tma_load_3d(st + F_OFF_BY, &tm.bq_halo[1], bar, x0, y0 - 4, k);
+  if (s <= L2S) {
+    const int m0 = z0 + (s - 1) * L2P, np = min(L2P, z0 + 7 - m0);
+    mbar_expect_tx(bar, np * TPP * TILE_BYTES);
+    for (int j = 0; j < np; ++j) {
+      tma_load_3d(st + (TPP * j) * TILE_FLOATS, &tm.tile[0], bar, x0, y0, m0 + j);
+      tma_load_3d(st + (TPP * j + 1) * TILE_FLOATS, &tm.tile[3], bar, x0, y0, m0 + j - 4);
+      if (HB) tma_load_3d(st + (TPP * j + 2) * TILE_FLOATS, &tm.bq_tile, bar, x0, y0, m0 + j - 4);
     }
+    return;
+  }
+  const int k = z0 + s - f_lead<HB>(), m = k + 7;
+  mbar_expect_tx(bar, (HB ? 3 : 2) * TILE_BYTES + (F_PB_FLOATS + (HB ? 2 : 1) * (F_VX_FLOATS + F_VY_FLOATS)) * 4 + (has_kc ? TILE_BYTES : 0));
+  tma_load_3d(st + F_OFF_PT, &tm.tile[0], bar, x0, y0, m);
+  tma_load_3d(st + F_OFF_VZ, &tm.tile[3], bar, x0, y0, m - 4);
+  if (HB) tma_load_3d(st + F_OFF_BZ, &tm.bq_tile, bar, x0, y0, m - 4);
+  tma_load_3d(st, &tm.p_box, bar, x0 - 8, y0 - 7, k);
+  tma_load_3d(st + F_OFF_VX, &tm.vx_halo, bar, x0 - 4, y0, k);
+  tma_load_3d(st + F_OFF_VY, &tm.vy_halo, bar, x0, y0 - 4, k);
+  if (has_kc) tma_load_3d(st + F_OFF_KC, &tm.tile[4], bar, x0, y0, k);
+  if (HB) {
+    tma_load_3d(st + F_OFF_BX, &tm.bq_halo[0], bar, x0 - 4, y0, k);
+    tma_load_3d(st + F_OFF_BY, &tm.bq_halo[1], bar, x0, y0 - 4, k);
   }
 }
 
@@ -136,6 +159,7 @@ struct MainState {
   long long goff;           // element offset of this thread's float4 in plane k of a field
   long long pox, poy;       // element offsets of plane k in the x / y slab psi arrays
   V4 nvx, npx, nvy, npy;    // psi_v / psi_p of plane k, loaded one iteration ahead (XS / YS items)
+  V4 nvz, npz;              // psi_vz of plane k+3 and psi_pz of plane k, loaded one iteration ahead (planes in a z slab)
   unsigned it, eit;
   bool pre;                 // the next stage's "full" phase was already seen complete by an early probe
 };
@@ -156,17 +180,27 @@ struct MainK {
 };
 
 // vz_new[kz] from the p ring (a0..a7 = p_old[kz-3 .. kz+4]); CPML in the z slabs; stored if this item owns the plane.
-template <bool HB, bool ZS>
+// z slab planes of local index v (0 <= v < nz): [0, zl) and [zh, nz)
+__device__ __forceinline__ bool in_z_slab(const DomainView& D, const MainK& K, int v) {
+  return (unsigned)(v - K.zl) >= (unsigned)(K.zh - K.zl) && (unsigned)v < (unsigned)D.nz;
+}
+// psi of the z slab (family fam) at plane v for this thread's float4, or zeros outside the slabs / for inactive threads
+__device__ __forceinline__ V4 load_psi_z(const DomainView& D, const MainK& K, int fam, int v) {
+  if (!(in_z_slab(D, K, v) && K.active)) return zero4();
+  const int sz = v < K.zl ? 0 : 1;
+  return ldg4(D.psi[fam][2][sz] + (long long)(v - D.ls[2][sz]) * D.plane + K.zrow);
+}
+template <bool HB, bool ZS, bool PRE>
 __device__ __forceinline__ V4 fused_vz(const DomainView& D, const OutSet& O, const MainK& K, const V4& a0, const V4& a1, const V4& a2,
                                        const V4& a3, const V4& a4, const V4& a5, const V4& a6, const V4& a7, V4 vz4, const V4& bz4, int kz,
-                                       long long goff_kz, bool own) {
+                                       long long goff_kz, bool own, const V4& psz_pre) {
   V4 dzv = diff_8(a4, a3, a5, a2, a6, a1, a7, a0);
   if (ZS && (unsigned)(kz - K.zl) >= (unsigned)(K.zh - K.zl) && (unsigned)kz < (unsigned)D.nz) {   // block-uniform: z slab
     const int sz = kz < K.zl ? 0 : 1;
-    const int gk = kz + D.oz;
     const long long poz = (long long)(kz - D.ls[2][sz]) * D.plane + K.zrow;
+    const int gk = kz + D.oz;
     const float ta = __ldg(D.tab[0][2][0] + gk), tb = __ldg(D.tab[0][2][1] + gk), tk = __ldg(D.tab[0][2][2] + gk);
-    V4 psz = K.active ? ldg4(D.psi[0][2][sz] + poz) : zero4();
+    V4 psz = PRE ? psz_pre : (K.active ? ldg4(D.psi[0][2][sz] + poz) : zero4());
     cpml4s(dzv, psz, ta, tb, tk);
     if (own) st4(O.psi[0][2][sz] + poz, psz);
   }
@@ -200,6 +234,13 @@ __device__ __forceinline__ void fused_plane(const DomainView& D, const OutSet& O
   if (YS) {
     psy = C.nvy; ppy = C.npy;
     if (K.in_y && k + 1 < K.z1) { C.nvy = ldg4(K.psi_in[0][1] + C.poy + K.stride_py); C.npy = ldg4(K.psi_in[1][1] + C.poy + K.stride_py); }
+  }
+  // z slabs: psi_vz of plane k+3 and psi_pz of plane k arrived during the previous iteration; start those of the next plane
+  V4 psz, ppz;
+  if (ZS) {
+    psz = C.nvz; ppz = C.npz;
+    C.nvz = load_psi_z(D, K, 0, k + 4);
+    C.npz = load_psi_z(D, K, 1, k + 1);
   }
   if (!C.pre) mbar_wait(&Q.full[slot], (C.it / FNS) & 1);
   C.pq[R] = ld4(st + F_OFF_PT + K.toff);                         // newest p_old plane k+7 replaces p_old[k-1]
@@ -248,17 +289,12 @@ __device__ __forceinline__ void fused_plane(const DomainView& D, const OutSet& O
   warp_arrive(&Q.efull[eb]);
 
   // ---- vz_new at kz+1/2 from p_old[kz-3 .. kz+4], then D-_z of the new vz ring
-  C.wq[R] = fused_vz<HB, ZS>(D, O, K, PQ(0), PQ(1), PQ(2), PQ(3), PQ(4), PQ(5), PQ(6), PQ(7), vz4, bz4, k + 3, C.goff + 3 * D.plane,
-                         K.active && k < K.zv_end);
+  C.wq[R] = fused_vz<HB, ZS, true>(D, O, K, PQ(0), PQ(1), PQ(2), PQ(3), PQ(4), PQ(5), PQ(6), PQ(7), vz4, bz4, k + 3, C.goff + 3 * D.plane,
+                               K.active && k < K.zv_end, psz);
   V4 dzp = diff_8(WQ(4), WQ(3), WQ(5), WQ(2), WQ(6), WQ(1), WQ(7), WQ(0));
-  V4 ppz;
   const bool pz = ZS && (unsigned)(k - K.zl) >= (unsigned)(K.zh - K.zl);    // block-uniform: plane k lies in a z slab
   const int szp = k < K.zl ? 0 : 1;
-  long long pozp = 0;
-  if (pz) {
-    pozp = (long long)(k - D.ls[2][szp]) * D.plane + K.zrow;
-    ppz = K.active ? ldg4(D.psi[1][2][szp] + pozp) : zero4();
-  }
+  const long long pozp = pz ? (long long)(k - D.ls[2][szp]) * D.plane + K.zrow : 0;
 
   // ---- pressure sub-update at plane k
   C.pre = mbar_test(&Q.full[(C.it + 1) % FNS], ((C.it + 1) / FNS) & 1);      // probe the next stage now, use the answer next iteration
@@ -303,6 +339,7 @@ __device__ __forceinline__ void fused_plane(const DomainView& D, const OutSet& O
 template <bool ZS, bool XS, bool YS, bool HB>
 __device__ __forceinline__ void fused_run(const DomainView& D, const OutSet& O, const float* smem, float* ebuf, const FusedBars& Q,
                                           const TabCache& T, const MainK& K, MainState<XS, YS>& C, int k, int kend) {
+  if (ZS && k < kend) { C.nvz = load_psi_z(D, K, 0, k + 3); C.npz = load_psi_z(D, K, 1, k); }
   for (; k < kend; ++k) {
 #pragma unroll
     for (int n = 0; n < 7; ++n) { C.pq[n] = C.pq[n + 1]; C.wq[n] = C.wq[n + 1]; }
@@ -350,37 +387,46 @@ __device__ __forceinline__ void fused_main_item(const DomainView& D, const OutSe
 #pragma unroll
   for (int n = 0; n < 8; ++n) { C.pq[n] = zero4(); C.wq[n] = zero4(); }
   constexpr int SF = f_stage_floats<HB>();
-  // lead-in 1: planes z0-7 .. z0-1 of p_old only fill the ring (canonical order: shifted, not renamed)
-  for (int m = z0 - 7; m < z0; ++m, ++C.it) {
+  // lead-in stage 0: the seven p tiles of planes z0-7 .. z0-1 fill the ring (entry 0 stays zero: it is the one shifted out first)
+  {
     const unsigned slot = C.it % FNS;
-    if (!C.pre) mbar_wait(&Q.full[slot], (C.it / FNS) & 1);
-    const V4 v = ld4(smem + slot * SF + F_OFF_PT + K.toff);
-    warp_arrive(&Q.empty[slot]);
-    C.pre = mbar_test(&Q.full[(C.it + 1) % FNS], ((C.it + 1) / FNS) & 1);
+    mbar_wait(&Q.full[slot], (C.it / FNS) & 1);
+    const float* st = smem + slot * SF + K.toff;
 #pragma unroll
-    for (int n = 0; n < 7; ++n) C.pq[n] = C.pq[n + 1];
-    C.pq[7] = v;
+    for (int j = 0; j < 7; ++j) C.pq[j + 1] = ld4(st + j * TILE_FLOATS);
+    warp_arrive(&Q.empty[slot]);
+    ++C.it;
   }
-  // lead-in 2: planes z0 .. z0+6 also produce vz_new[z0-4 .. z0+2] (the first four belong to the z chunk below)
-  for (int m = z0; m < z0 + 7; ++m, ++C.it) {
-    const unsigned slot = C.it % FNS;
-    const float* st = smem + slot * SF;
-    if (!C.pre) mbar_wait(&Q.full[slot], (C.it / FNS) & 1);
-    const V4 v = ld4(st + F_OFF_PT + K.toff);
-    V4 vz4 = ld4(st + F_OFF_VZ + K.toff);
-    V4 bz4;
-    if (HB) bz4 = ld4(st + F_OFF_BZ + K.toff);
-    warp_arrive(&Q.empty[slot]);
-    C.pre = mbar_test(&Q.full[(C.it + 1) % FNS], ((C.it + 1) / FNS) & 1);
+  // lead-in stages 1 .. L2S: planes m = z0 .. z0+6 also produce vz_new[z0-4 .. z0+2] (the first four belong to the z chunk below)
+  {
+    constexpr int L2P = f_lead2_planes<HB>(), L2S = f_lead2_stages<HB>(), TPP = f_lead2_tiles<HB>();
+    int m = z0;
+    for (int b = 0; b < L2S; ++b, ++C.it) {
+      const unsigned slot = C.it % FNS;
+      mbar_wait(&Q.full[slot], (C.it / FNS) & 1);
+      const float* st = smem + slot * SF + K.toff;
 #pragma unroll
-    for (int n = 0; n < 7; ++n) C.pq[n] = C.pq[n + 1];
-    C.pq[7] = v;
-    const int kz = m - 4;                                            // planes z0 .. z0+2 are this item's own
-    vz4 = fused_vz<HB, true>(D, O, K, C.pq[0], C.pq[1], C.pq[2], C.pq[3], C.pq[4], C.pq[5], C.pq[6], C.pq[7], vz4, bz4, kz,
-                       K.zrow + (long long)kz * D.plane, K.active && kz >= z0 && kz < z1);
+      for (int j = 0; j < L2P; ++j) {
+        if (m < z0 + 7) {                                              // block-uniform
+          const V4 v = ld4(st + (TPP * j) * TILE_FLOATS);
+          V4 vz4 = ld4(st + (TPP * j + 1) * TILE_FLOATS);
+          V4 bz4;
+          if (HB) bz4 = ld4(st + (TPP * j + 2) * TILE_FLOATS);
 #pragma unroll
-    for (int n = 0; n < 7; ++n) C.wq[n] = C.wq[n + 1];
-    C.wq[7] = vz4;
+          for (int n = 0; n < 7; ++n) C.pq[n] = C.pq[n + 1];
+          C.pq[7] = v;
+          const int kz = m - 4;                                        // planes z0 .. z0+2 are this item's own
+          vz4 = fused_vz<HB, true, false>(D, O, K, C.pq[0], C.pq[1], C.pq[2], C.pq[3], C.pq[4], C.pq[5], C.pq[6], C.pq[7], vz4, bz4, kz,
+                                    K.zrow + (long long)kz * D.plane, K.active && kz >= z0 && kz < z1, vz4);
+#pragma unroll
+          for (int n = 0; n < 7; ++n) C.wq[n] = C.wq[n + 1];
+          C.wq[7] = vz4;
+          ++m;
+        }
+      }
+      warp_arrive(&Q.empty[slot]);
+    }
+    C.pre = false;
   }
   // now pq[n] = p_old[z0-1+n], wq[n] = vz_new[z0-5+n]: entry 0 of both rings is the oldest
   if (XS && K.in_x) { C.nvx = ldg4(K.psi_in[0][0] + C.pox); C.npx = ldg4(K.psi_in[1][0] + C.pox); }
@@ -428,7 +474,7 @@ __device__ __forceinline__ void fused_halo(const DomainView& D, float* smem, flo
   long long pox = sx >= 0 ? psi_index(D, 0, sx, xx, jx, z0) : 0;
   const long long stride_px = sx >= 0 ? (long long)D.ny * D.ln[0][sx] : 0;
   const int xcol = side ? TX + 4 : 0;                        // the strip's first column in the table cache
-  const int m_begin = z0 - 7, m_end = z1 + 7;
+  const int m_begin = z0 + 7 - f_lead<HB>(), m_end = z1 + 7;      // the first f_lead() stages are the batched lead-in: wait and release only
   V4 npsy = zero4(), npsx = zero4();
   if (sy >= 0) npsy = ldg4(D.psi[0][1][sy] + poy);
   if (sx >= 0) npsx = ldg4(D.psi[0][0][sx] + pox);
@@ -535,7 +581,7 @@ __global__ void __launch_bounds__(FNT, 1) step_fused(const __grid_constant__ TMa
     while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) {
       fill_tab_cache(D, tabc, x0, y0);
       fused_halo<HB>(D, smem, ebuf, Q, tabc, it, eit, warp - FW_MAIN, x0, y0, z0, z1);
-      it += z1 - z0 + F_LEAD;
+      it += z1 - z0 + f_lead<HB>();
       eit += z1 - z0;
     }
   } else {
@@ -543,12 +589,12 @@ __global__ void __launch_bounds__(FNT, 1) step_fused(const __grid_constant__ TMa
     const bool has_kc = D.kc != nullptr;
     const bool producer = threadIdx.x == FNW * 32;
     while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) {
-      const int niter = z1 - z0 + F_LEAD;
+      const int niter = z1 - z0 + f_lead<HB>();
       if (producer) {
         for (int s = 0; s < niter; ++s) {
           const unsigned slot = (it + s) % FNS;
           if (s >= FNS) mbar_wait(&Q.empty[slot], ((it + s - FNS) / FNS) & 1);      // every consumer warp released the stage
-          fused_issue<HB>(tm, smem, Q.full, slot, z0 - 7 + s, x0, y0, z0, has_kc);
+          fused_issue<HB>(tm, smem, Q.full, slot, s, x0, y0, z0, has_kc);
         }
       }
       it += niter;
