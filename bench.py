@@ -11,6 +11,8 @@ configs 3 and 2 are timed in the same run and carried under "other_workloads".  
 5 times (CUDA events, barrier + synchronize on both sides); value / ms_per_step are the median repeat (the paper
 reports medians), min and max are printed beside it.  One process per GPU; N > 1 runs N independent
 replicas (the path does not shard: DESIGN.md "Multi-GPU"), value = points of all ranks / max-over-ranks time.
+Every workload is timed from a counter-based random state (random mantissas draw the most power, and the loop runs at the
+board's power cap); the config's own initial state (zero fields + its sources) is timed beside it as "state_zero_fields".
 Prints ONE JSON line on rank 0.
 """
 import argparse

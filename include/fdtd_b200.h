@@ -63,7 +63,8 @@ enum {
                         /* per point instead of 48), the single-GPU form of the enlarged ghost of P:42 (a     */
                         /* ghost of 2r = 8 cells per step, recomputed in x and y, streamed in z).  Out of      */
                         /* place: the workspace holds two copies of the fields and psi.  Same bits as AUTO.   */
-                        /* Needs FDTD_WALL, total Nx % 4 == 0 and an even substeps_per_exchange.              */
+                        /* Needs FDTD_WALL; in subdomain mode also a total Nx % 4 == 0 and an even            */
+                        /* substeps_per_exchange.                                                              */
 };
 
 /* Problem statement and Table 2 as one plain-data block. */
@@ -175,8 +176,9 @@ int fdtd_coeffs(float out_host[4]);
 
 /* The kernel family this context runs: FDTD_KERNEL_AUTO (the TMA-tiled kernels), FDTD_KERNEL_REF or FDTD_KERNEL_FUSED.
  * A context created with FDTD_KERNEL_AUTO runs the much slower one-thread-per-point FDTD_KERNEL_REF kernels when the
- * tiled ones do not apply (FDTD_PERIODIC, or a total Nx that is not a multiple of 4: they move whole float4s); this
- * call is how a caller finds out. */
+ * tiled ones do not apply (FDTD_PERIODIC, FDTD_PRECISION_FP64, or subdomain mode with a total Nx that is not a multiple
+ * of 4: the halo copies move whole float4s); this call is how a caller finds out.  A monolithic grid of any Nx runs the
+ * tiled kernels. */
 int fdtd_kernel_in_use(const fdtd_ctx* ctx);
 
 /* time_block >= 2: plane-steps computed (ghost planes included) and plane-steps owned since fdtd_create, into

@@ -72,8 +72,6 @@ struct Geometry {
   std::string why;
 };
 
-long long n_total_x(const fdtd_params& P) { return (long long)P.n_interior[0] + P.cpml[0] + P.cpml[1]; }
-
 Geometry make_geometry(const fdtd_params& P) {
   Geometry G;
   auto bad = [&](const char* w) { G.valid = false; G.why = w; return G; };
@@ -88,8 +86,7 @@ Geometry make_geometry(const fdtd_params& P) {
   if (!(P.dx > 0.0) || !(P.dt > 0.0)) return bad("dx and dt must be positive");
   if (P.boundary != FDTD_WALL && P.boundary != FDTD_PERIODIC) return bad("unknown boundary");
   if (P.kernel < FDTD_KERNEL_AUTO || P.kernel > FDTD_KERNEL_FUSED) return bad("unknown kernel selector");
-  if (P.kernel == FDTD_KERNEL_FUSED && (P.boundary == FDTD_PERIODIC || (n_total_x(P) % 4) != 0))
-    return bad("FDTD_KERNEL_FUSED needs WALL boundaries and a total Nx that is a multiple of 4");
+  if (P.kernel == FDTD_KERNEL_FUSED && P.boundary == FDTD_PERIODIC) return bad("FDTD_KERNEL_FUSED needs WALL boundaries");
   if (P.density != FDTD_DENSITY_UNIFORM && P.density != FDTD_DENSITY_ARRAY) return bad("unknown density selector");
   if (P.medium != FDTD_MEDIUM_ARRAY && P.medium != FDTD_MEDIUM_UNIFORM) return bad("unknown medium selector");
   if (P.precision != FDTD_PRECISION_FP32 && P.precision != FDTD_PRECISION_FP64) return bad("unknown precision selector");
@@ -111,6 +108,7 @@ Geometry make_geometry(const fdtd_params& P) {
     if (P.boundary == FDTD_PERIODIC) return bad("subdomain mode needs WALL boundaries");
     if (G.msub < 1 || G.ghost < 4 * G.msub) return bad("ghost must be >= 4 * substeps_per_exchange");
     if (P.kernel == FDTD_KERNEL_FUSED && (G.msub % 2)) return bad("the fused step advances two sub-updates: substeps_per_exchange must be even");
+    if (P.kernel == FDTD_KERNEL_FUSED && (G.gn[0] % 4)) return bad("FDTD_KERNEL_FUSED in subdomain mode needs a total Nx that is a multiple of 4");
     for (int a = 0; a < 3; ++a) {
       if (G.gn[a] % G.nd[a]) return bad("total grid not divisible by decomp");
       if (G.gn[a] / G.nd[a] < G.ghost) return bad("ghost deeper than a subdomain");
@@ -767,10 +765,12 @@ fdtd_ctx* fdtd_create(const fdtd_params* P) {
   c->P = *P; c->G = G; c->L = L;
   c->ws = (char*)P->workspace;
   c->stream = (cudaStream_t)P->stream;
-  // the tiled kernels move whole float4s: they need Nx % 4 == 0; other grids take the reference kernels
+  // The tiled kernels move whole float4s.  A monolithic grid of any Nx takes them (the last float4 of a row reaches into the
+  // row's padding, which nothing reads: TMA bounds are the grid's); the halo copies of the subdomain mode need Nx % 4 == 0.
   c->fp64 = P->precision == FDTD_PRECISION_FP64;
   c->es = c->fp64 ? 8 : 4;
-  c->use_ref = P->kernel == FDTD_KERNEL_REF || P->boundary == FDTD_PERIODIC || (G.gn[0] % 4) != 0 || c->fp64;
+  const bool subdomains = G.nd[0] * G.nd[1] * G.nd[2] > 1;
+  c->use_ref = P->kernel == FDTD_KERNEL_REF || P->boundary == FDTD_PERIODIC || (subdomains && (G.gn[0] % 4) != 0) || c->fp64;
   c->fused = P->kernel == FDTD_KERNEL_FUSED;      // make_geometry has checked that the tiled path applies
   cudaError_t e;
   if ((e = cudaSetDevice(P->device)) != cudaSuccess) return fail(c, e, "cudaSetDevice");

@@ -171,7 +171,8 @@ struct MainK {
   int z1, zv_end;           // last output plane + 1; vz planes >= zv_end belong to the next z chunk
   int zl, zh;               // z slabs: local planes [0, zl) and [zh, nz)
   int kz_pin;               // vz planes >= kz_pin take a zero update coefficient (pinned last half node R3, and planes above the grid)
-  float B, Bx3, By, kc0;
+  float B, By, kc0;
+  int pinx;                 // element of this thread's float4 that is the pinned last half node of x (R3), 4: none
   bool active, in_x, in_y, has_kc;
   int sxs, sys;             // slab side (0 / 1) of this thread's columns / row when in_x / in_y
   long long stride_px, stride_py, zrow;
@@ -273,11 +274,11 @@ __device__ __forceinline__ void fused_plane(const DomainView& D, const OutSet& O
   if (HB) {
 #pragma unroll
     for (int e = 0; e < 4; ++e) {
-      vx4.v[e] = upd(vx4.v[e], (e == 3 && K.Bx3 == 0.f) ? 0.f : bx4.v[e], dxv.v[e]);
+      vx4.v[e] = upd(vx4.v[e], e >= K.pinx ? 0.f : bx4.v[e], dxv.v[e]);
       vy4.v[e] = upd(vy4.v[e], K.By == 0.f ? 0.f : by4.v[e], dyv.v[e]);
     }
   } else {
-    vx4 = upd4(vx4, K.B, K.B, K.Bx3, dxv);
+    vx4 = upd4_pin(vx4, K.B, K.pinx, dxv);
     vy4 = upd4(vy4, K.By, K.By, K.By, dyv);
   }
   if (K.active) { st4(O.f[1] + C.goff, vx4); st4(O.f[2] + C.goff, vy4); }
@@ -359,7 +360,7 @@ __device__ __forceinline__ void fused_main_item(const DomainView& D, const OutSe
   K.kc0 = D.kc0;
   K.active = (i < D.nx) && (j < D.ny);
   K.B = K.active ? D.b0 : 0.f;
-  K.Bx3 = (i + 3 + D.ox) == D.gn[0] - 1 ? 0.f : (HB ? 1.f : K.B);     // pinned last half node (R3); HB: only the zero matters
+  K.pinx = pinned_x_element(i + D.ox, D.gn[0]);
   K.By = (j + D.oy) == D.gn[1] - 1 ? 0.f : (HB ? 1.f : K.B);
   K.kz_pin = min(D.gn[2] - 1 - D.oz, D.nz);
   K.zrow = (long long)j * D.pitch + i;
@@ -467,7 +468,7 @@ __device__ __forceinline__ void fused_halo(const DomainView& D, float* smem, flo
   const int xx = side ? x0 + TX : x0 - 4, jx = y0 + row;
   const bool valid_x = do_x && xx >= 0 && xx < D.nx && jx < D.ny;
   const float Bvx = valid_x ? D.b0 : 0.f;
-  const float Bx3 = (xx + 3 + D.ox) == D.gn[0] - 1 ? 0.f : Bvx;
+  const int pinx = pinned_x_element(xx + D.ox, D.gn[0]);
   const int boff_x = (row + 7) * BW + (side ? TX + 8 : 4);
   const int exo = row * HW + (side ? TX + 4 : 0);
   const int sx = valid_x ? slab_side(D, 0, xx) : -1;
@@ -524,9 +525,9 @@ __device__ __forceinline__ void fused_halo(const DomainView& D, float* smem, flo
         }
         if (HB) {
 #pragma unroll
-          for (int e = 0; e < 4; ++e) vx4.v[e] = upd(vx4.v[e], (Bvx == 0.f || (e == 3 && Bx3 == 0.f)) ? 0.f : bx4.v[e], dxv.v[e]);
+          for (int e = 0; e < 4; ++e) vx4.v[e] = upd(vx4.v[e], (Bvx == 0.f || e >= pinx) ? 0.f : bx4.v[e], dxv.v[e]);
         } else {
-          vx4 = upd4(vx4, Bvx, Bvx, Bx3, dxv);
+          vx4 = upd4_pin(vx4, Bvx, pinx, dxv);
         }
       }
       const unsigned eb = eit % E_BUFS;

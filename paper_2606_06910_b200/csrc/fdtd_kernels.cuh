@@ -315,6 +315,18 @@ __device__ __forceinline__ V4 diff_8(const V4& h1, const V4& l1, const V4& h2, c
 __device__ __forceinline__ V4 upd4(const V4& f, float c01, float c2, float c3, const V4& d) {
   return join2(mad2(pk(-c01, -c01), lo2(d), lo2(f)), mad2(pk(-c2, -c3), hi2(d), hi2(f)));
 }
+// The pinned last half node of the x axis (R3) inside a float4 that starts at global column g: its element index, or 4
+// if the float4 does not hold it.  When Nx is a multiple of 4 it is always element 3 (the fast path of the callers).
+__device__ __forceinline__ int pinned_x_element(int g, int gnx) {
+  const unsigned e = (unsigned)(gnx - 1 - g);
+  return e < 4u ? (int)e : 4;
+}
+// f - c d for four points with the coefficient zeroed from element `pin` on (4: none): the pinned half node keeps its
+// value, and the elements behind it lie outside the grid, where v is 0 (R4) — they arrive as zeros (TMA bounds) and must stay
+// zeros, because the single-pass step hands vx_new to the neighbouring columns through shared memory.
+__device__ __forceinline__ V4 upd4_pin(const V4& f, float c, int pin, const V4& d) {
+  return join2(mad2(pk(pin <= 0 ? -0.f : -c, pin <= 1 ? -0.f : -c), lo2(d), lo2(f)), mad2(pk(pin <= 2 ? -0.f : -c, pin <= 3 ? -0.f : -c), hi2(d), hi2(f)));
+}
 __device__ __forceinline__ void cpml4(V4& d, V4& ps, const V4& a, const V4& b, const V4& ik) {
   const float2 p0 = mad2(lo2(b), lo2(ps), mul2(lo2(a), lo2(d))), p1 = mad2(hi2(b), hi2(ps), mul2(hi2(a), hi2(d)));
   d = join2(mad2(lo2(d), lo2(ik), p0), mad2(hi2(d), hi2(ik), p1));
@@ -400,7 +412,7 @@ __device__ __forceinline__ void v_item(const TMaps& tm, const DomainView& D, flo
   const int poff = (ty + 3) * HW + 4 * tx + 4;      // own float4 inside the p halo tile
   const int toff = ty * TX + 4 * tx;                // own float4 inside a plain tile
   // pinned last half nodes: zero coefficient
-  const float Bx3 = (i + 3 + D.ox) == D.gn[0] - 1 ? 0.f : B;
+  const int pinx = pinned_x_element(i + D.ox, D.gn[0]);
   const float By = (j + D.oy) == D.gn[1] - 1 ? 0.f : B;
   // CPML: block-uniform "does this item touch an x / y slab", per-thread "is my float4 / row inside one"
   const bool any_x = touches(D, 0, x0, x0 + TX), any_y = touches(D, 1, y0, y0 + TY);
@@ -461,7 +473,6 @@ __device__ __forceinline__ void v_item(const TMaps& tm, const DomainView& D, flo
     if (xy) {
       if (any_x) {
         if (sx >= 0) {
-          const int gi = i + D.ox;
           cpml4(dxv, psx, ld4(T.x[0] + 4 * tx), ld4(T.x[1] + 4 * tx), ld4(T.x[2] + 4 * tx));
           st4(ppx, psx);
           ppx += stride_px;
@@ -469,24 +480,23 @@ __device__ __forceinline__ void v_item(const TMaps& tm, const DomainView& D, flo
       }
       if (any_y) {
         if (sy >= 0) {
-          const int gj = j + D.oy;
           cpml4s(dyv, psy, T.y[0][ty], T.y[1][ty], T.y[2][ty]);
           st4(ppy, psy);
           ppy += stride_py;
         }
       }
       if (HB) {
-        const bool lastx = (i + 3 + D.ox) == D.gn[0] - 1, lasty = (j + D.oy) == D.gn[1] - 1;
+        const bool lasty = (j + D.oy) == D.gn[1] - 1;
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
-          vx4.v[e] = upd(vx4.v[e], (e == 3 && lastx) ? 0.f : bx4.v[e], dxv.v[e]);
+          vx4.v[e] = upd(vx4.v[e], e >= pinx ? 0.f : bx4.v[e], dxv.v[e]);
           vy4.v[e] = upd(vy4.v[e], lasty ? 0.f : by4.v[e], dyv.v[e]);
         }
         gbx += D.plane;
         gby += D.plane;
       } else {
-        vx4.v[0] = upd(vx4.v[0], B, dxv.v[0]); vx4.v[1] = upd(vx4.v[1], B, dxv.v[1]);
-        vx4.v[2] = upd(vx4.v[2], B, dxv.v[2]); vx4.v[3] = upd(vx4.v[3], Bx3, dxv.v[3]);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) vx4.v[e] = upd(vx4.v[e], e >= pinx ? 0.f : B, dxv.v[e]);
 #pragma unroll
         for (int e = 0; e < 4; ++e) vy4.v[e] = upd(vy4.v[e], By, dyv.v[e]);
       }
@@ -641,7 +651,6 @@ __device__ __forceinline__ void p_item(const TMaps& tm, const DomainView& D, flo
       V4 dzv = diff_8(q4, q3, q5, q2, q6, q1, q7, q0);
       if (any_x) {
         if (sx >= 0) {
-          const int gi = i + D.ox;
           cpml4(dxv, psx, ld4(T.x[0] + 4 * tx), ld4(T.x[1] + 4 * tx), ld4(T.x[2] + 4 * tx));
           st4(ppx, psx);
           ppx += stride_px;
@@ -649,7 +658,6 @@ __device__ __forceinline__ void p_item(const TMaps& tm, const DomainView& D, flo
       }
       if (any_y) {
         if (sy >= 0) {
-          const int gj = j + D.oy;
           cpml4s(dyv, psy, T.y[0][ty], T.y[1][ty], T.y[2][ty]);
           st4(ppy, psy);
           ppy += stride_py;

@@ -85,15 +85,16 @@ def test_config1_full_parity(B, kernel):
 @pytest.mark.parametrize("kernel", [1, 0, 2])
 @pytest.mark.parametrize("shape,cpml", [
     ((70, 45, 37), (5, 9, 0, 7, 6, 0)),        # ragged tiles in x and y, faces without a layer, unequal thickness
-    ((133, 18, 21), (12, 12, 4, 4, 8, 8)),     # nx not a multiple of 4: the library routes this to the reference kernels
+    ((133, 18, 21), (12, 12, 4, 4, 8, 8)),     # nx = 157, not a multiple of 4: the last float4 of a row is partial, the pinned half node is element 0
+    ((130, 18, 21), (12, 12, 4, 4, 8, 8)),     # nx = 154: pinned element 1
+    ((47, 18, 21), (0, 12, 4, 4, 8, 8)),       # nx = 59: pinned element 2, a single ragged tile, no low x layer
+    ((129, 18, 21), (12, 0, 4, 4, 8, 8)),      # nx = 141: pinned element 0, no high x layer
     ((124, 18, 21), (12, 12, 4, 4, 8, 8)),     # three x tiles, the last one ragged (148 = 2*64 + 20)
     ((24, 20, 150), (0, 0, 0, 0, 10, 10)),     # long in z: several z chunks
 ])
 def test_random_state_ragged_parity(B, kernel, shape, cpml):
     """All four fields random (counter-based generator on both sides), heterogeneous c, 6 steps."""
     tot = tuple(shape[a] + cpml[2 * a] + cpml[2 * a + 1] for a in range(3))
-    if kernel == 2 and tot[0] % 4:
-        pytest.skip("FDTD_KERNEL_FUSED needs Nx % 4 == 0 (fdtd_create refuses, see test_errors_are_reported_not_fatal)")
     rng = np.random.default_rng(11)
     c = (1.0 + 0.3 * rng.random(tot[::-1])).astype(np.float32)
     kw = dict(dt=0.4 / 1.3, cpml_alpha_max=math.pi * inputs.F0, cpml_c_ref=1.3)
@@ -229,8 +230,6 @@ def test_heterogeneous_density_parity(B, kernel, shape, cpml):
     """SURVEY NEXT-3 (reading R6): rho(x) and c(x) both heterogeneous; dt/(rho_bar dx) at the half nodes.
     All three kernel families, the single-pass step included (three more TMA tiles per stage)."""
     tot = tuple(shape[a] + cpml[2 * a] + cpml[2 * a + 1] for a in range(3))
-    if kernel == 2 and tot[0] % 4:
-        pytest.skip("FDTD_KERNEL_FUSED needs Nx % 4 == 0")
     rng = np.random.default_rng(3)
     c = (1.0 + 0.3 * rng.random(tot[::-1])).astype(np.float32)
     rho = (0.8 + 0.7 * rng.random(tot[::-1])).astype(np.float32)
@@ -348,7 +347,7 @@ def test_errors_are_reported_not_fatal(B):
         sim.set_model(None, rho)
     sim.step(1)
     sim.destroy()
-    for bad in (dict(n_interior=(18, 16, 16)), dict(n_interior=(16,) * 3, boundary=B.FDTD_PERIODIC)):
+    for bad in (dict(n_interior=(18, 16, 16), decomp=(1, 2, 1), ghost=8, substeps=2), dict(n_interior=(16,) * 3, boundary=B.FDTD_PERIODIC)):
         with pytest.raises(B.FdtdError):                            # the fused step refuses what it cannot run
             B.Fdtd(bad.pop("n_interior"), dt=0.4, kernel=B.FDTD_KERNEL_FUSED, **bad)
 
@@ -413,7 +412,13 @@ def test_kernel_in_use_reports_the_reference_fallback_and_uniform_medium_refuses
     sim = B.Fdtd((64, 16, 16), dt=0.4)
     assert sim.kernel_in_use() == B.FDTD_KERNEL_AUTO
     sim.destroy()
-    sim = B.Fdtd((66, 16, 16), dt=0.4)                         # Nx % 4 != 0: AUTO falls back, and says so
+    sim = B.Fdtd((66, 16, 16), dt=0.4)                         # a monolithic grid of any Nx takes the tiled kernels
+    assert sim.kernel_in_use() == B.FDTD_KERNEL_AUTO
+    sim.destroy()
+    sim = B.Fdtd((66, 16, 16), dt=0.4, decomp=(1, 2, 1), ghost=4, substeps=1)   # subdomain mode with Nx % 4 != 0: AUTO falls back, and says so
+    assert sim.kernel_in_use() == B.FDTD_KERNEL_REF
+    sim.destroy()
+    sim = B.Fdtd((16, 16, 16), dt=0.4, boundary=B.FDTD_PERIODIC)
     assert sim.kernel_in_use() == B.FDTD_KERNEL_REF
     sim.destroy()
     sim = B.Fdtd((64, 16, 16), dt=0.4, kernel=B.FDTD_KERNEL_FUSED, medium=B.FDTD_MEDIUM_UNIFORM)
