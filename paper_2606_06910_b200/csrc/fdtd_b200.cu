@@ -306,6 +306,32 @@ int make_tmap(EncodeTiledFn enc, CUtensorMap* m, float* base, const DomainView& 
   return FDTD_OK;
 }
 
+// x / y slab psi as tensors for the single-pass step's stage: the x slab [nz][ny][w] with a PXW x TY box, the y slab
+// [nz][rows][pitch] with a TX x TY box.
+int make_tmap_psi(EncodeTiledFn enc, CUtensorMap* m, float* base, int d0, int d1, int d2, long long row_stride, int bw) {
+  cuuint64_t dims[3] = {(cuuint64_t)d0, (cuuint64_t)d1, (cuuint64_t)d2};
+  cuuint64_t strides[2] = {(cuuint64_t)row_stride * 4, (cuuint64_t)row_stride * 4 * (cuuint64_t)d1};
+  cuuint32_t box[3] = {(cuuint32_t)bw, (cuuint32_t)TY, 1};
+  cuuint32_t estr[3] = {1, 1, 1};
+  CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                   CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { set_err("cuTensorMapEncodeTiled (psi) failed with CUresult " + std::to_string((int)r)); return FDTD_ECUDA; }
+  return FDTD_OK;
+}
+
+// Can the x / y slab psi of this domain go through the TMA stage of step_fused?  The x slabs must fit the staged box and no
+// tile may touch both slabs of an axis (a tile's box comes from one slab array).
+bool psi_tma_ok(const DomainView& v) {
+  for (int s = 0; s < 2; ++s) if (v.ln[0][s] > PXW) return false;
+  const int tile[2] = {TX, TY}, n[2] = {v.nx, v.ny};
+  for (int a = 0; a < 2; ++a) {
+    if (v.ln[a][0] == 0 || v.ln[a][1] == 0) continue;
+    for (int t0 = 0; t0 < n[a]; t0 += tile[a])
+      if (t0 < v.ls[a][0] + v.ln[a][0] && t0 + tile[a] > v.ls[a][1]) return false;
+  }
+  return true;
+}
+
 // Persistent launch plan: grid = resident CTAs; items = tiles x z-chunks with enough items per CTA for balance.
 int plan_launch(fdtd_ctx* c, const void* kernel, int smem, int* grid, int threads = NT) {
   int per_sm = 0, sms = 148;
@@ -329,6 +355,8 @@ void plan_items(Domain& d, int grid) {
   S.zchunk = (v.nz + n - 1) / n;
   S.nzc = (v.nz + S.zchunk - 1) / S.zchunk;
   S.nitems = (int)(tiles * S.nzc);
+  S.table = nullptr;
+  S.psi_tma = 0;
 }
 
 // step_fused items: every item pays a lead-in of 14 planes (batched into 3 - 4 pipeline stages), so chunks are long.
@@ -371,6 +399,15 @@ void plan_items_fused(Domain& d, int grid, std::vector<int4>& table) {
   S.zchunk = (int)zc;
   S.nzc = (int)zb.size() - 1;
   S.nitems = (int)table.size();
+  S.psi_tma = (v.bq[0] == nullptr && psi_tma_ok(v)) ? 1 : 0;
+}
+
+// The three builds of the single-pass step: 1 = density arrays, 2 = uniform density with the x / y slab psi through the TMA
+// stage (when the domain's slabs allow it, psi_tma_ok), 0 = uniform density with psi by global loads.
+void launch_step_fused(int grid, cudaStream_t stream, const TMaps& tm, const DomainView& vin, const OutSet& O, const Sched& S) {
+  if (vin.bq[0]) step_fused<1><<<grid, FNT, f_smem_bytes<1>(), stream>>>(tm, vin, O, S);
+  else if (S.psi_tma) step_fused<2><<<grid, FNT, f_smem_bytes<2>(), stream>>>(tm, vin, O, S);
+  else step_fused<0><<<grid, FNT, f_smem_bytes<0>(), stream>>>(tm, vin, O, S);
 }
 
 // One fused time step of one domain: state v.f / v.psi -> d.alt, then the two are swapped.
@@ -378,8 +415,7 @@ int launch_fused(fdtd_ctx* c, Domain& d) {
   Sched S = d.sched_f;
   S.counter = d.counters + 2 + d.fused_parity;
   S.other = d.counters + 2 + (1 - d.fused_parity);
-  if (d.v.bq[0]) step_fused<true><<<std::min(c->grid_f, S.nitems), FNT, f_smem_bytes<true>(), c->stream>>>(d.tm, d.v, d.alt, S);
-  else step_fused<false><<<std::min(c->grid_f, S.nitems), FNT, f_smem_bytes<false>(), c->stream>>>(d.tm, d.v, d.alt, S);
+  launch_step_fused(std::min(c->grid_f, S.nitems), c->stream, d.tm, d.v, d.alt, S);
   c->launches++;
   CK(cudaGetLastError());
   d.fused_parity ^= 1;
@@ -439,8 +475,7 @@ int do_time_block(fdtd_ctx* c) {
     S.nitems = L.nitems;
     S.counter = d.counters + 2 + d.fused_parity;
     S.other = d.counters + 2 + (1 - d.fused_parity);
-    if (vin.bq[0]) step_fused<true><<<std::min(c->grid_f, S.nitems), FNT, f_smem_bytes<true>(), c->stream>>>(*tm, vin, O, S);
-    else step_fused<false><<<std::min(c->grid_f, S.nitems), FNT, f_smem_bytes<false>(), c->stream>>>(*tm, vin, O, S);
+    launch_step_fused(std::min(c->grid_f, S.nitems), c->stream, *tm, vin, O, S);
     c->launches++;
     CK(cudaGetLastError());
     d.fused_parity ^= 1;
@@ -853,7 +888,7 @@ fdtd_ctx* fdtd_create(const fdtd_params* P) {
       d.counters = (unsigned int*)(c->ws + ld.counters);
       if (!c->use_ref) {
         float* kcbase = L.has_kc ? (float*)(c->ws + ld.kc) : (float*)(c->ws + ld.f[0]);   // no Kc slot: the map is never used
-        auto make_maps = [&](TMaps& tm, float* const f[4]) -> int {
+        auto make_maps = [&](TMaps& tm, float* const f[4], float* const psi[2][3][2]) -> int {
           float* tile_base[5] = {f[0], f[1], f[2], f[3], kcbase};
           int bad = make_tmap(enc, &tm.p_halo, f[0], v, HW, VH) || make_tmap(enc, &tm.vx_halo, f[1], v, HW, TY) ||
                     make_tmap(enc, &tm.vy_halo, f[2], v, TX, PH) || make_tmap(enc, &tm.p_box, f[0], v, BW, BH);
@@ -862,21 +897,27 @@ fdtd_ctx* fdtd_create(const fdtd_params* P) {
             bad = make_tmap(enc, &tm.bq_halo[0], (float*)(c->ws + ld.bq[0]), v, HW, TY) ||
                   make_tmap(enc, &tm.bq_halo[1], (float*)(c->ws + ld.bq[1]), v, TX, PH) ||
                   make_tmap(enc, &tm.bq_tile, (float*)(c->ws + ld.bq[2]), v, TX, TY);
+          if (c->fused && psi)
+            for (int fam = 0; fam < 2 && !bad; ++fam)
+              for (int s = 0; s < 2 && !bad; ++s) {
+                if (v.ln[0][s] > 0) bad = make_tmap_psi(enc, &tm.psi_x[fam][s], psi[fam][0][s], v.ln[0][s], v.ny, v.nz, v.ln[0][s], PXW);
+                if (v.ln[1][s] > 0 && !bad) bad = make_tmap_psi(enc, &tm.psi_y[fam][s], psi[fam][1][s], v.nx, v.ln[1][s], v.nz, v.pitch, TX);
+              }
           return bad;
         };
-        int bad = make_maps(d.tm, v.f);
+        int bad = make_maps(d.tm, v.f, v.psi);
         if (c->fused && !bad) {
           for (int f = 0; f < 4; ++f) d.alt.f[f] = (float*)(c->ws + ld.f2[f]);
           for (int fam = 0; fam < 2; ++fam)
             for (int a = 0; a < 3; ++a)
               for (int s = 0; s < 2; ++s) d.alt.psi[fam][a][s] = (float*)(c->ws + ld.psi2[fam][a][s]);
-          bad = make_maps(d.tm_alt, d.alt.f);
+          bad = make_maps(d.tm_alt, d.alt.f, d.alt.psi);
           for (int x = 0; x < (P->time_block > 2 ? 2 : (P->time_block > 1 ? 1 : 0)) && !bad; ++x) {
             for (int f = 0; f < 4; ++f) d.xs[x].f[f] = (float*)(c->ws + ld.fx[x][f]);
             for (int fam = 0; fam < 2; ++fam)
               for (int a = 0; a < 3; ++a)
                 for (int s = 0; s < 2; ++s) d.xs[x].psi[fam][a][s] = (float*)(c->ws + ld.psix[x][fam][a][s]);
-            bad = make_maps(d.tm_xs[x], d.xs[x].f);
+            bad = make_maps(d.tm_xs[x], d.xs[x].f, d.xs[x].psi);
           }
         }
         if (bad) { delete c; return nullptr; }
@@ -895,11 +936,12 @@ fdtd_ctx* fdtd_create(const fdtd_params* P) {
         plan_launch(c, (const void*)update_p_tiled, P_SMEM_BYTES, &c->grid_p)) { delete c; return nullptr; }
     for (auto& d : c->doms) plan_items(d, std::min(c->grid_v, c->grid_p));
     if (c->fused) {
-      if ((e = cudaFuncSetAttribute(step_fused<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, f_smem_bytes<false>())) != cudaSuccess ||
-          (e = cudaFuncSetAttribute(step_fused<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, f_smem_bytes<true>())) != cudaSuccess)
+      if ((e = cudaFuncSetAttribute(step_fused<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, f_smem_bytes<0>())) != cudaSuccess ||
+          (e = cudaFuncSetAttribute(step_fused<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, f_smem_bytes<1>())) != cudaSuccess ||
+          (e = cudaFuncSetAttribute(step_fused<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, f_smem_bytes<2>())) != cudaSuccess)
         return fail(c, e, "cudaFuncSetAttribute(step_fused)");
       const bool hb = P->density == FDTD_DENSITY_ARRAY;
-      if (plan_launch(c, hb ? (const void*)step_fused<true> : (const void*)step_fused<false>, hb ? f_smem_bytes<true>() : f_smem_bytes<false>(),
+      if (plan_launch(c, hb ? (const void*)step_fused<1> : (const void*)step_fused<2>, hb ? f_smem_bytes<1>() : f_smem_bytes<2>(),
                       &c->grid_f, FNT)) { delete c; return nullptr; }
       for (size_t k = 0; k < c->doms.size(); ++k) {
         Domain& d = c->doms[k];

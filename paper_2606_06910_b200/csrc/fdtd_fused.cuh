@@ -42,10 +42,10 @@ constexpr int FNS = 4;                           // TMA ring stages
 // stage the lead-in ran at the latency of four TMA round trips per four planes (980 cycles per plane, measured).  So the
 // lead-in planes are batched: stage 0 of an item holds the seven p tiles of planes z0-7 .. z0-1, the next L2S stages hold L2P
 // planes each of (p tile of plane m, vz tile of plane m-4 [, dt/(rho_bar dx) of vz]) for m = z0 .. z0+6.
-template <bool HB> __host__ __device__ constexpr int f_lead2_planes() { return HB ? 3 : 4; }      // planes per lead-in-2 stage
-template <bool HB> __host__ __device__ constexpr int f_lead2_stages() { return HB ? 3 : 2; }      // 3+3+1 or 4+3 planes
-template <bool HB> __host__ __device__ constexpr int f_lead2_tiles() { return HB ? 3 : 2; }       // tiles per lead-in-2 plane
-template <bool HB> __host__ __device__ constexpr int f_lead() { return 1 + f_lead2_stages<HB>(); } // stages before the first output plane
+template <int V> __host__ __device__ constexpr int f_lead2_planes() { return V == 1 ? 3 : 4; }      // planes per lead-in-2 stage
+template <int V> __host__ __device__ constexpr int f_lead2_stages() { return V == 1 ? 3 : 2; }      // 3+3+1 or 4+3 planes
+template <int V> __host__ __device__ constexpr int f_lead2_tiles() { return V == 1 ? 3 : 2; }       // tiles per lead-in-2 plane
+template <int V> __host__ __device__ constexpr int f_lead() { return 1 + f_lead2_stages<V>(); } // stages before the first output plane
 constexpr int BW = TX + 16;                      // p box: columns x0-8 .. x0+TX+7
 constexpr int BH = TY + 14;                      // p box: rows    y0-7 .. y0+TY+6
 constexpr int EVY_ROWS = TY + 8;                 // vy_new exchange rows y0-4 .. y0+TY+3 (the last one is never read)
@@ -60,17 +60,21 @@ constexpr int F_OFF_KC = F_OFF_VY + F_VY_FLOATS;
 constexpr int F_OFF_BX = F_OFF_KC + TILE_FLOATS; // HB only
 constexpr int F_OFF_BY = F_OFF_BX + F_VX_FLOATS;
 constexpr int F_OFF_BZ = F_OFF_BY + F_VY_FLOATS;
-template <bool HB> __host__ __device__ constexpr int f_stage_floats() {
-  return HB ? F_OFF_BZ + TILE_FLOATS : (F_OFF_BX > 8 * TILE_FLOATS ? F_OFF_BX : 8 * TILE_FLOATS);   // a lead-in-2 stage holds 4 x 2 tiles
-}
-static_assert(7 * TILE_FLOATS <= f_stage_floats<false>() && 9 * TILE_FLOATS <= f_stage_floats<true>(), "lead-in batches must fit a stage");
+// x / y slab psi of plane k through the stage (uniform density only: the density-array stage has no room for it):
+// [psi_vx box PXW x TY | psi_px | psi_vy tile | psi_py tile] behind the 8 tiles a lead-in-2 stage holds
+constexpr int F_OFF_PSXV = 8 * TILE_FLOATS, F_OFF_PSXP = F_OFF_PSXV + PXW * TY, F_OFF_PSYV = F_OFF_PSXP + PXW * TY, F_OFF_PSYP = F_OFF_PSYV + TILE_FLOATS;
+static_assert(F_OFF_BX <= 8 * TILE_FLOATS && (PXW * TY * 4) % 128 == 0, "stage layout");
+// kernel variant V: 0 = uniform density, x / y slab psi by global loads; 1 = density arrays (HB); 2 = uniform density, x / y
+// slab psi through the stage (PT)
+template <int V> __host__ __device__ constexpr int f_stage_floats() { return V == 1 ? F_OFF_BZ + TILE_FLOATS : (V == 2 ? F_OFF_PSYP + TILE_FLOATS : 8 * TILE_FLOATS); }
+static_assert(8 * TILE_FLOATS <= f_stage_floats<0>() && 9 * TILE_FLOATS <= f_stage_floats<1>() && 8 * TILE_FLOATS <= f_stage_floats<2>(), "lead-in batches must fit a stage");
 constexpr int E_OFF_VY = F_VX_FLOATS;            // exchange buffer: [vx_new 16 x 72 | vy_new 24 x 64]
 constexpr int E_FLOATS = F_VX_FLOATS + TX * EVY_ROWS;
 constexpr int E_BUFS = 3;                        // three exchange buffers: the halo warps may run two planes ahead of the main warps
-template <bool HB> __host__ __device__ constexpr int f_smem_bytes() { return (FNS * f_stage_floats<HB>() + E_BUFS * E_FLOATS) * 4; }
+template <int V> __host__ __device__ constexpr int f_smem_bytes() { return (FNS * f_stage_floats<V>() + E_BUFS * E_FLOATS) * 4; }
 static_assert((F_PB_FLOATS * 4) % 128 == 0 && (F_VX_FLOATS * 4) % 128 == 0 && (F_VY_FLOATS * 4) % 128 == 0 && (E_FLOATS * 4) % 128 == 0,
               "TMA destinations must stay 128-B aligned");
-static_assert(f_smem_bytes<true>() <= 227 * 1024 - 4096, "stage ring + exchange buffers + static shared memory must fit one SM");
+static_assert(f_smem_bytes<1>() <= 227 * 1024 - 4096 && f_smem_bytes<2>() <= 227 * 1024 - 4096, "stage ring + exchange buffers + static shared memory must fit one SM");
 
 // The "out" state of a fused step (same layout as the DomainView's own arrays, which are the "in" state).
 struct OutSet {
@@ -112,12 +116,13 @@ __device__ __forceinline__ void warp_arrive(uint64_t* bar) {
 }
 
 // Stage s of an item: s = 0 and 1 .. L2S are the batched lead-in stages, s >= f_lead() carries output plane k = z0 + s - f_lead().
-template <bool HB>
+template <int V>
 __device__ __forceinline__ void fused_issue(const TMaps& tm, float* smem, uint64_t* full, unsigned slot, int s, int x0, int y0, int z0,
-                                            bool has_kc) {
-  constexpr int L2P = f_lead2_planes<HB>(), L2S = f_lead2_stages<HB>(), TPP = f_lead2_tiles<HB>();
+                                            bool has_kc, const DomainView& D) {
+  constexpr bool HB = V == 1;
+  constexpr int L2P = f_lead2_planes<V>(), L2S = f_lead2_stages<V>(), TPP = f_lead2_tiles<V>();
   uint64_t* bar = &full[slot];
-  float* st = smem + slot * f_stage_floats<HB>();
+  float* st = smem + slot * f_stage_floats<V>();
   if (s == 0) {
     mbar_expect_tx(bar, 7 * TILE_BYTES);
 #pragma unroll
@@ -134,8 +139,29 @@ __device__ __forceinline__ void fused_issue(const TMaps& tm, float* smem, uint64
     }
     return;
   }
-  const int k = z0 + s - f_lead<HB>(), m = k + 7;
-  mbar_expect_tx(bar, (HB ? 3 : 2) * TILE_BYTES + (F_PB_FLOATS + (HB ? 2 : 1) * (F_VX_FLOATS + F_VY_FLOATS)) * 4 + (has_kc ? TILE_BYTES : 0));
+  const int k = z0 + s - f_lead<V>(), m = k + 7;
+  // the x / y slab this tile touches, if its psi goes through the stage (recomputed per stage from the kernel parameters: the
+  // producer lane has 32 registers, and whatever it spills it reloads behind a tensor copy, at a thousand cycles a load)
+  int sxt = -1, syt = -1;
+  if (V == 2) {
+#pragma unroll
+    for (int side = 0; side < 2; ++side) {
+      if (D.ln[0][side] > 0 && x0 < D.ls[0][side] + D.ln[0][side] && x0 + TX > D.ls[0][side]) sxt = side;
+      if (D.ln[1][side] > 0 && y0 < D.ls[1][side] + D.ln[1][side] && y0 + TY > D.ls[1][side]) syt = side;
+    }
+  }
+  mbar_expect_tx(bar, (HB ? 3 : 2) * TILE_BYTES + (F_PB_FLOATS + (HB ? 2 : 1) * (F_VX_FLOATS + F_VY_FLOATS)) * 4 + (has_kc ? TILE_BYTES : 0) +
+                          (sxt >= 0 ? 2 * PXW * TY * 4 : 0) + (syt >= 0 ? 2 * TILE_BYTES : 0));
+  if (V == 2 && sxt >= 0) {         // psi_vx, psi_px of plane k: the slab's columns from the tile's first one on, this tile's rows
+    const int cx0 = max(x0, D.ls[0][sxt]) - D.ls[0][sxt];
+    tma_load_3d(st + F_OFF_PSXV, &tm.psi_x[0][sxt], bar, cx0, y0, k);
+    tma_load_3d(st + F_OFF_PSXP, &tm.psi_x[1][sxt], bar, cx0, y0, k);
+  }
+  if (V == 2 && syt >= 0) {         // psi_vy, psi_py of plane k: this tile's columns, 16 slab rows from the tile's first row (outside the slab: zero fill)
+    const int cy0 = y0 - D.ls[1][syt];
+    tma_load_3d(st + F_OFF_PSYV, &tm.psi_y[0][syt], bar, x0, cy0, k);
+    tma_load_3d(st + F_OFF_PSYP, &tm.psi_y[1][syt], bar, x0, cy0, k);
+  }
   tma_load_3d(st + F_OFF_PT, &tm.tile[0], bar, x0, y0, m);
   tma_load_3d(st + F_OFF_VZ, &tm.tile[3], bar, x0, y0, m - 4);
   if (HB) tma_load_3d(st + F_OFF_BZ, &tm.bq_tile, bar, x0, y0, m - 4);
@@ -152,7 +178,8 @@ __device__ __forceinline__ void fused_issue(const TMaps& tm, float* smem, uint64
 // ---- main warps: the tile's own points ------------------------------------------------------------------
 // Everything a main thread keeps over one item.  The two z queues are arrays that are only ever indexed with
 // compile-time constants, so they live in registers.
-template <bool XS, bool YS>
+// XS / YS: 0 = the item touches no x / y slab, 1 = psi by global loads one plane ahead, 2 = psi through the TMA stage
+template <int XS, int YS>
 struct MainState {
   V4 pq[8];                 // p_old ring:  logical entry n (after the push of plane k) = p_old[k+n]
   V4 wq[8];                 // vz_new ring: logical entry n (after the push of plane k) = vz_new[k-4+n]
@@ -173,6 +200,7 @@ struct MainK {
   int kz_pin;               // vz planes >= kz_pin take a zero update coefficient (pinned last half node R3, and planes above the grid)
   float B, By, kc0;
   int pinx;                 // element of this thread's float4 that is the pinned last half node of x (R3), 4: none
+  int psxo;                 // own float4 in the staged x-slab psi box (XS == 2)
   bool active, in_x, in_y, has_kc;
   int sxs, sys;             // slab side (0 / 1) of this thread's columns / row when in_x / in_y
   long long stride_px, stride_py, zrow;
@@ -191,10 +219,11 @@ __device__ __forceinline__ V4 load_psi_z(const DomainView& D, const MainK& K, in
   const int sz = v < K.zl ? 0 : 1;
   return ldg4(D.psi[fam][2][sz] + (long long)(v - D.ls[2][sz]) * D.plane + K.zrow);
 }
-template <bool HB, bool ZS, bool PRE>
+template <int V, bool ZS, bool PRE>
 __device__ __forceinline__ V4 fused_vz(const DomainView& D, const OutSet& O, const MainK& K, const V4& a0, const V4& a1, const V4& a2,
                                        const V4& a3, const V4& a4, const V4& a5, const V4& a6, const V4& a7, V4 vz4, const V4& bz4, int kz,
                                        long long goff_kz, bool own, const V4& psz_pre) {
+  constexpr bool HB = V == 1;
   V4 dzv = diff_8(a4, a3, a5, a2, a6, a1, a7, a0);
   if (ZS && (unsigned)(kz - K.zl) >= (unsigned)(K.zh - K.zl) && (unsigned)kz < (unsigned)D.nz) {   // block-uniform: z slab
     const int sz = kz < K.zl ? 0 : 1;
@@ -219,20 +248,21 @@ __device__ __forceinline__ V4 fused_vz(const DomainView& D, const OutSet& O, con
 
 // One steady-state iteration: output plane k (m = k+7, kz = k+3).  R = position of the oldest ring entry on entry.
 // ZS = this plane or its vz plane may lie in a z slab (the lean instantiation carries no z-slab code at all).
-template <int R, bool ZS, bool XS, bool YS, bool HB>
+template <int R, bool ZS, int XS, int YS, int V>
 __device__ __forceinline__ void fused_plane(const DomainView& D, const OutSet& O, const float* smem, float* ebuf, const FusedBars& Q,
                                             const TabCache& T, const MainK& K, MainState<XS, YS>& C, int k) {
+  constexpr bool HB = V == 1;
 #define PQ(n) C.pq[(R + 1 + (n)) & 7]
 #define WQ(n) C.wq[(R + 1 + (n)) & 7]
   const unsigned slot = C.it % FNS;
-  const float* st = smem + slot * f_stage_floats<HB>();
+  const float* st = smem + slot * f_stage_floats<V>();
   // psi of plane k arrived during the previous iteration; start the loads of plane k+1 now
   V4 psx, psy, ppx, ppy;
-  if (XS) {
+  if (XS == 1) {
     psx = C.nvx; ppx = C.npx;
     if (K.in_x && k + 1 < K.z1) { C.nvx = ldg4(K.psi_in[0][0] + C.pox + K.stride_px); C.npx = ldg4(K.psi_in[1][0] + C.pox + K.stride_px); }
   }
-  if (YS) {
+  if (YS == 1) {
     psy = C.nvy; ppy = C.npy;
     if (K.in_y && k + 1 < K.z1) { C.nvy = ldg4(K.psi_in[0][1] + C.poy + K.stride_py); C.npy = ldg4(K.psi_in[1][1] + C.poy + K.stride_py); }
   }
@@ -256,6 +286,8 @@ __device__ __forceinline__ void fused_plane(const DomainView& D, const OutSet& O
   const V4 kc4 = K.has_kc ? ld4(st + F_OFF_KC + K.toff) : splat4(K.kc0);
   V4 bx4, by4, bz4;
   if (HB) { bx4 = ld4(st + F_OFF_BX + K.exo); by4 = ld4(st + F_OFF_BY + 4 * TX + K.toff); bz4 = ld4(st + F_OFF_BZ + K.toff); }
+  if (XS == 2 && K.in_x) { psx = ld4(st + F_OFF_PSXV + K.psxo); ppx = ld4(st + F_OFF_PSXP + K.psxo); }
+  if (YS == 2 && K.in_y) { psy = ld4(st + F_OFF_PSYV + K.toff); ppy = ld4(st + F_OFF_PSYP + K.toff); }
   warp_arrive(&Q.empty[slot]);
 
   // ---- velocity sub-update at plane k
@@ -290,7 +322,7 @@ __device__ __forceinline__ void fused_plane(const DomainView& D, const OutSet& O
   warp_arrive(&Q.efull[eb]);
 
   // ---- vz_new at kz+1/2 from p_old[kz-3 .. kz+4], then D-_z of the new vz ring
-  C.wq[R] = fused_vz<HB, ZS, true>(D, O, K, PQ(0), PQ(1), PQ(2), PQ(3), PQ(4), PQ(5), PQ(6), PQ(7), vz4, bz4, k + 3, C.goff + 3 * D.plane,
+  C.wq[R] = fused_vz<V, ZS, true>(D, O, K, PQ(0), PQ(1), PQ(2), PQ(3), PQ(4), PQ(5), PQ(6), PQ(7), vz4, bz4, k + 3, C.goff + 3 * D.plane,
                                K.active && k < K.zv_end, psz);
   V4 dzp = diff_8(WQ(4), WQ(3), WQ(5), WQ(2), WQ(6), WQ(1), WQ(7), WQ(0));
   const bool pz = ZS && (unsigned)(k - K.zl) >= (unsigned)(K.zh - K.zl);    // block-uniform: plane k lies in a z slab
@@ -337,20 +369,21 @@ __device__ __forceinline__ void fused_plane(const DomainView& D, const OutSet& O
 // per plane (56 register moves).  Renaming instead of moving needs the body unrolled 8x (or 4x / 2x with a rotation per
 // group), and every unrolled form measured slower than this one (8x: 2.06 instead of 1.44 ms at 552^3, 4x: 1.51, 2x: 1.50):
 // the body must stay resident in the instruction cache, and the kernel is not bound by issue slots.
-template <bool ZS, bool XS, bool YS, bool HB>
+template <bool ZS, int XS, int YS, int V>
 __device__ __forceinline__ void fused_run(const DomainView& D, const OutSet& O, const float* smem, float* ebuf, const FusedBars& Q,
                                           const TabCache& T, const MainK& K, MainState<XS, YS>& C, int k, int kend) {
   if (ZS && k < kend) { C.nvz = load_psi_z(D, K, 0, k + 3); C.npz = load_psi_z(D, K, 1, k); }
   for (; k < kend; ++k) {
 #pragma unroll
     for (int n = 0; n < 7; ++n) { C.pq[n] = C.pq[n + 1]; C.wq[n] = C.wq[n + 1]; }
-    fused_plane<7, ZS, XS, YS, HB>(D, O, smem, ebuf, Q, T, K, C, k);       // writes the newest entries at index 7
+    fused_plane<7, ZS, XS, YS, V>(D, O, smem, ebuf, Q, T, K, C, k);       // writes the newest entries at index 7
   }
 }
 
-template <bool XS, bool YS, bool HB>
+template <int XS, int YS, int V>
 __device__ __forceinline__ void fused_main_item(const DomainView& D, const OutSet& O, const float* smem, float* ebuf, const FusedBars& Q,
                                              const TabCache& T, unsigned& it_io, unsigned& eit_io, int x0, int y0, int z0, int z1) {
+  constexpr bool HB = V == 1;
   const int tid = threadIdx.x;
   MainK K;
   K.tx = tid & 15; K.ty = tid >> 4;
@@ -373,6 +406,7 @@ __device__ __forceinline__ void fused_main_item(const DomainView& D, const OutSe
   const int sy = (YS && K.active) ? slab_side(D, 1, j) : -1;
   K.in_x = sx >= 0; K.in_y = sy >= 0;
   K.sxs = max(sx, 0); K.sys = max(sy, 0);
+  K.psxo = K.in_x ? K.ty * PXW + (i - max(x0, D.ls[0][K.sxs])) : 0;
   K.stride_px = K.in_x ? (long long)D.ny * D.ln[0][K.sxs] : 0;
   K.stride_py = K.in_y ? (long long)D.ln[1][K.sys] * D.pitch : 0;
 #pragma unroll
@@ -387,7 +421,7 @@ __device__ __forceinline__ void fused_main_item(const DomainView& D, const OutSe
   C.goff = K.zrow + (long long)z0 * D.plane;
 #pragma unroll
   for (int n = 0; n < 8; ++n) { C.pq[n] = zero4(); C.wq[n] = zero4(); }
-  constexpr int SF = f_stage_floats<HB>();
+  constexpr int SF = f_stage_floats<V>();
   // lead-in stage 0: the seven p tiles of planes z0-7 .. z0-1 fill the ring (entry 0 stays zero: it is the one shifted out first)
   {
     const unsigned slot = C.it % FNS;
@@ -400,7 +434,7 @@ __device__ __forceinline__ void fused_main_item(const DomainView& D, const OutSe
   }
   // lead-in stages 1 .. L2S: planes m = z0 .. z0+6 also produce vz_new[z0-4 .. z0+2] (the first four belong to the z chunk below)
   {
-    constexpr int L2P = f_lead2_planes<HB>(), L2S = f_lead2_stages<HB>(), TPP = f_lead2_tiles<HB>();
+    constexpr int L2P = f_lead2_planes<V>(), L2S = f_lead2_stages<V>(), TPP = f_lead2_tiles<V>();
     int m = z0;
     for (int b = 0; b < L2S; ++b, ++C.it) {
       const unsigned slot = C.it % FNS;
@@ -417,7 +451,7 @@ __device__ __forceinline__ void fused_main_item(const DomainView& D, const OutSe
           for (int n = 0; n < 7; ++n) C.pq[n] = C.pq[n + 1];
           C.pq[7] = v;
           const int kz = m - 4;                                        // planes z0 .. z0+2 are this item's own
-          vz4 = fused_vz<HB, true, false>(D, O, K, C.pq[0], C.pq[1], C.pq[2], C.pq[3], C.pq[4], C.pq[5], C.pq[6], C.pq[7], vz4, bz4, kz,
+          vz4 = fused_vz<V, true, false>(D, O, K, C.pq[0], C.pq[1], C.pq[2], C.pq[3], C.pq[4], C.pq[5], C.pq[6], C.pq[7], vz4, bz4, kz,
                                     K.zrow + (long long)kz * D.plane, K.active && kz >= z0 && kz < z1, vz4);
 #pragma unroll
           for (int n = 0; n < 7; ++n) C.wq[n] = C.wq[n + 1];
@@ -430,24 +464,25 @@ __device__ __forceinline__ void fused_main_item(const DomainView& D, const OutSe
     C.pre = false;
   }
   // now pq[n] = p_old[z0-1+n], wq[n] = vz_new[z0-5+n]: entry 0 of both rings is the oldest
-  if (XS && K.in_x) { C.nvx = ldg4(K.psi_in[0][0] + C.pox); C.npx = ldg4(K.psi_in[1][0] + C.pox); }
-  if (YS && K.in_y) { C.nvy = ldg4(K.psi_in[0][1] + C.poy); C.npy = ldg4(K.psi_in[1][1] + C.poy); }
+  if (XS == 1 && K.in_x) { C.nvx = ldg4(K.psi_in[0][0] + C.pox); C.npx = ldg4(K.psi_in[1][0] + C.pox); }
+  if (YS == 1 && K.in_y) { C.nvy = ldg4(K.psi_in[0][1] + C.poy); C.npy = ldg4(K.psi_in[1][1] + C.poy); }
   // z range of the item = [z0, za) + [za, zb) + [zb, z1): only the outer two can touch a z slab (plane k or vz plane k+3)
   const int za = min(max(K.zl, z0), z1), zb = min(max(K.zh - 3, za), z1);
-  fused_run<true, XS, YS, HB>(D, O, smem, ebuf, Q, T, K, C, z0, za);
-  fused_run<false, XS, YS, HB>(D, O, smem, ebuf, Q, T, K, C, za, zb);
-  fused_run<true, XS, YS, HB>(D, O, smem, ebuf, Q, T, K, C, zb, z1);
+  fused_run<true, XS, YS, V>(D, O, smem, ebuf, Q, T, K, C, z0, za);
+  fused_run<false, XS, YS, V>(D, O, smem, ebuf, Q, T, K, C, za, zb);
+  fused_run<true, XS, YS, V>(D, O, smem, ebuf, Q, T, K, C, zb, z1);
   it_io = C.it; eit_io = C.eit;
 }
 
 // ---- halo warps: the redundantly computed ghost of the tile, never stored to global memory ----------------
 // Warp hw (0..3) computes vy_new on two of the rows y0-4..y0-1, y0+TY..y0+TY+2 (16 float4 units per row; the eighth
 // row slot is idle); warp 3 also computes vx_new on the strips x0-4..x0-1 and x0+TX..x0+TX+3 (rows y0..y0+TY-1).
-template <bool HB>
+template <int V>
 __device__ __forceinline__ void fused_halo(const DomainView& D, float* smem, float* ebuf, const FusedBars& Q, const TabCache& T, unsigned it,
                                            unsigned eit, int hw, int x0, int y0, int z0, int z1) {
+  constexpr bool HB = V == 1;
   const int lane = threadIdx.x & 31;
-  constexpr int SF = f_stage_floats<HB>();
+  constexpr int SF = f_stage_floats<V>();
   // vy unit of this lane
   const int r = 2 * hw + (lane >> 4), c = lane & 15;
   const int jy = r < 4 ? y0 - 4 + r : y0 + TY + (r - 4), iy = x0 + 4 * c;
@@ -475,7 +510,7 @@ __device__ __forceinline__ void fused_halo(const DomainView& D, float* smem, flo
   long long pox = sx >= 0 ? psi_index(D, 0, sx, xx, jx, z0) : 0;
   const long long stride_px = sx >= 0 ? (long long)D.ny * D.ln[0][sx] : 0;
   const int xcol = side ? TX + 4 : 0;                        // the strip's first column in the table cache
-  const int m_begin = z0 + 7 - f_lead<HB>(), m_end = z1 + 7;      // the first f_lead() stages are the batched lead-in: wait and release only
+  const int m_begin = z0 + 7 - f_lead<V>(), m_end = z1 + 7;      // the first f_lead() stages are the batched lead-in: wait and release only
   V4 npsy = zero4(), npsx = zero4();
   if (sy >= 0) npsy = ldg4(D.psi[0][1][sy] + poy);
   if (sx >= 0) npsx = ldg4(D.psi[0][0][sx] + pox);
@@ -544,12 +579,12 @@ __device__ __forceinline__ void fused_halo(const DomainView& D, float* smem, flo
   }
 }
 
-template <bool HB>
+template <int V>
 __global__ void __launch_bounds__(FNT, 1) step_fused(const __grid_constant__ TMaps tm, const __grid_constant__ DomainView D,
                                                      const __grid_constant__ OutSet O, const __grid_constant__ Sched S) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   float* smem = reinterpret_cast<float*>(smem_raw);
-  float* ebuf = smem + FNS * f_stage_floats<HB>();
+  float* ebuf = smem + FNS * f_stage_floats<V>();
   __shared__ __align__(8) uint64_t bars[2 * FNS + E_BUFS];
   __shared__ int s_item;
   __shared__ __align__(16) TabCache tabc;
@@ -572,17 +607,21 @@ __global__ void __launch_bounds__(FNT, 1) step_fused(const __grid_constant__ TMa
     while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) {
       fill_tab_cache(D, tabc, x0, y0);
       const bool xs = touches(D, 0, x0, x0 + TX), ys = touches(D, 1, y0, y0 + TY);      // block-uniform
-      if (!xs && !ys) fused_main_item<false, false, HB>(D, O, smem, ebuf, Q, tabc, it, eit, x0, y0, z0, z1);
-      else if (xs && !ys) fused_main_item<true, false, HB>(D, O, smem, ebuf, Q, tabc, it, eit, x0, y0, z0, z1);
-      else if (!xs) fused_main_item<false, true, HB>(D, O, smem, ebuf, Q, tabc, it, eit, x0, y0, z0, z1);
-      else fused_main_item<true, true, HB>(D, O, smem, ebuf, Q, tabc, it, eit, x0, y0, z0, z1);
+      // Few instantiations per kernel: with seven plane-body variants in one kernel ptxas spilled 1.3 KB in the main warps
+      // (with two, nothing).  Variant 2 runs every slab item through one instantiation; a tile that touches only an x slab
+      // has in_y false in every thread and skips the y code by a uniform branch.
+      if (!xs && !ys) fused_main_item<0, 0, V>(D, O, smem, ebuf, Q, tabc, it, eit, x0, y0, z0, z1);
+      else if constexpr (V == 2) fused_main_item<2, 2, V>(D, O, smem, ebuf, Q, tabc, it, eit, x0, y0, z0, z1);
+      else if (xs && !ys) fused_main_item<1, 0, V>(D, O, smem, ebuf, Q, tabc, it, eit, x0, y0, z0, z1);
+      else if (!xs) fused_main_item<0, 1, V>(D, O, smem, ebuf, Q, tabc, it, eit, x0, y0, z0, z1);
+      else fused_main_item<1, 1, V>(D, O, smem, ebuf, Q, tabc, it, eit, x0, y0, z0, z1);
     }
   } else if (warp < FNW) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(F_REGS_HALO));
     while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) {
       fill_tab_cache(D, tabc, x0, y0);
-      fused_halo<HB>(D, smem, ebuf, Q, tabc, it, eit, warp - FW_MAIN, x0, y0, z0, z1);
-      it += z1 - z0 + f_lead<HB>();
+      fused_halo<V>(D, smem, ebuf, Q, tabc, it, eit, warp - FW_MAIN, x0, y0, z0, z1);
+      it += z1 - z0 + f_lead<V>();
       eit += z1 - z0;
     }
   } else {
@@ -590,12 +629,12 @@ __global__ void __launch_bounds__(FNT, 1) step_fused(const __grid_constant__ TMa
     const bool has_kc = D.kc != nullptr;
     const bool producer = threadIdx.x == FNW * 32;
     while (next_item(S, &s_item, x0, y0, z0, z1, D.nz)) {
-      const int niter = z1 - z0 + f_lead<HB>();
+      const int niter = z1 - z0 + f_lead<V>();
       if (producer) {
         for (int s = 0; s < niter; ++s) {
           const unsigned slot = (it + s) % FNS;
           if (s >= FNS) mbar_wait(&Q.empty[slot], ((it + s - FNS) / FNS) & 1);      // every consumer warp released the stage
-          fused_issue<HB>(tm, smem, Q.full, slot, s, x0, y0, z0, has_kc);
+          fused_issue<V>(tm, smem, Q.full, slot, s, x0, y0, z0, has_kc, D);
         }
       }
       it += niter;

@@ -261,7 +261,10 @@ struct TMaps {
   CUtensorMap p_box;      // p,  box (TX+16) x (TY+14)   (step_fused)
   CUtensorMap bq_halo[2]; // dt/(rho_bar dx) of vx, box HW x TY; of vy, box TX x PH   (step_fused<true>)
   CUtensorMap bq_tile;    // dt/(rho_bar dx) of vz, box TX x TY                         (step_fused<true>)
+  CUtensorMap psi_x[2][2]; // x-slab psi [family][side] as (w, ny, nz), box PXW x TY   (step_fused<false>, psi through the stage)
+  CUtensorMap psi_y[2][2]; // y-slab psi [family][side] as (nx, rows, nz), box TX x TY (step_fused<false>, psi through the stage)
 };
+constexpr int PXW = 40;    // widest x slab (columns, multiple of 4) whose psi goes through the TMA stage
 
 // Work decomposition of one launch (same for both sub-updates of a domain).
 struct Sched {
@@ -270,6 +273,8 @@ struct Sched {
   unsigned int* counter;       // this launch's work counter
   unsigned int* other;         // the counter of the next launch on this domain: reset here
   const int4* table;           // optional: item -> (x0, y0, z0, z1) in the order they are handed out (nullptr: tile-major decode)
+  int psi_tma;                 // step_fused: the x / y slab psi of the main warps arrives through the TMA stage (host-checked: slabs
+                               // at most PXW columns wide, no tile touches both slabs of an axis, no density arrays)
 };
 
 // Four consecutive x values held in registers; moved as one 128-bit access.
