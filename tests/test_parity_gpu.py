@@ -91,6 +91,9 @@ def test_config1_full_parity(B, kernel):
     ((129, 18, 21), (12, 0, 4, 4, 8, 8)),      # nx = 141: pinned element 0, no high x layer
     ((124, 18, 21), (12, 12, 4, 4, 8, 8)),     # three x tiles, the last one ragged (148 = 2*64 + 20)
     ((24, 20, 150), (0, 0, 0, 0, 10, 10)),     # long in z: several z chunks
+    ((30, 10, 20), (3, 3, 3, 3, 4, 4)),        # one tile touches both slabs of x and of y: the single-pass step loads psi itself (build 0)
+    ((100, 20, 20), (44, 41, 4, 4, 4, 4)),     # x layers wider than the staged psi box (40 columns): build 0 as well
+    ((100, 40, 20), (36, 33, 18, 17, 4, 4)),   # x slabs of 36 columns, y slabs of more than a tile: psi through the stage (build 2)
 ])
 def test_random_state_ragged_parity(B, kernel, shape, cpml):
     """All four fields random (counter-based generator on both sides), heterogeneous c, 6 steps."""
