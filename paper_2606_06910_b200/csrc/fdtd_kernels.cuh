@@ -332,15 +332,23 @@ __device__ __forceinline__ int pinned_x_element(int g, int gnx) {
 __device__ __forceinline__ V4 upd4_pin(const V4& f, float c, int pin, const V4& d) {
   return join2(mad2(pk(pin <= 0 ? -0.f : -c, pin <= 1 ? -0.f : -c), lo2(d), lo2(f)), mad2(pk(pin <= 2 ? -0.f : -c, pin <= 3 ? -0.f : -c), hi2(d), hi2(f)));
 }
+// An exact packed product for the CPML terms: fma(a, b, -0) is the rounded product bit for bit (signed zeros, subnormals,
+// infinities and NaNs included), and an FFMA2 cannot be folded into the FADD2 that consumes it the way ptxas folds a packed
+// multiply.  The -0 comes from constant memory, so that the compiler cannot see its value and turn the fma back into a
+// multiply.  Used in the slab code only: it halves the multiplies of a CPML term (three products per point), which is what a
+// slab plane pays on top of an interior one; in the stencil sums it changed no measured time (profiles/r02_ncu_step_fused.md).
+__constant__ float2 c_negzero2 = {-0.0f, -0.0f};
+__device__ __forceinline__ float2 mul2x(float2 a, float2 b) { return __ffma2_rn(a, b, c_negzero2); }
+__device__ __forceinline__ float2 mad2x(float2 a, float2 b, float2 c) { return __fadd2_rn(mul2x(a, b), c); }
 __device__ __forceinline__ void cpml4(V4& d, V4& ps, const V4& a, const V4& b, const V4& ik) {
-  const float2 p0 = mad2(lo2(b), lo2(ps), mul2(lo2(a), lo2(d))), p1 = mad2(hi2(b), hi2(ps), mul2(hi2(a), hi2(d)));
-  d = join2(mad2(lo2(d), lo2(ik), p0), mad2(hi2(d), hi2(ik), p1));
+  const float2 p0 = mad2x(lo2(b), lo2(ps), mul2x(lo2(a), lo2(d))), p1 = mad2x(hi2(b), hi2(ps), mul2x(hi2(a), hi2(d)));
+  d = join2(mad2x(lo2(d), lo2(ik), p0), mad2x(hi2(d), hi2(ik), p1));
   ps = join2(p0, p1);
 }
 __device__ __forceinline__ void cpml4s(V4& d, V4& ps, float a, float b, float ik) {
   const float2 a2 = pk(a, a), b2 = pk(b, b), k2 = pk(ik, ik);
-  const float2 p0 = mad2(b2, lo2(ps), mul2(a2, lo2(d))), p1 = mad2(b2, hi2(ps), mul2(a2, hi2(d)));
-  d = join2(mad2(lo2(d), k2, p0), mad2(hi2(d), k2, p1));
+  const float2 p0 = mad2x(b2, lo2(ps), mul2x(a2, lo2(d))), p1 = mad2x(b2, hi2(ps), mul2x(a2, hi2(d)));
+  d = join2(mad2x(lo2(d), k2, p0), mad2x(hi2(d), k2, p1));
   ps = join2(p0, p1);
 }
 
