@@ -386,9 +386,15 @@ void plan_items_fused(Domain& d, int grid, std::vector<int4>& table) {
   };
   struct Item { double cost; int4 t; };
   std::vector<Item> items;
+  // Inside one cost class the order is x fastest.  On wide grids (16 or more tiles per row) the rows go in pairs, y fastest
+  // inside a pair, so that a tile's y neighbour is its neighbour in the list as well and its y halo is found in L2 (DRAM
+  // reads of a 1600^3 step: 97.6 -> 88 GB with bands of 4 rows; 0.6 % of the capped step with pairs, which cost narrow grids
+  // 1 %: there the rows are close in the list anyway).
+  const int band = S.ntx >= 16 ? 2 : 1;
   for (size_t c = 0; c + 1 < zb.size(); ++c)
-    for (int ty = 0; ty < S.nty; ++ty)
-      for (int tx = 0; tx < S.ntx; ++tx) {
+    for (int b0 = 0; b0 < S.nty; b0 += band)
+      for (int tx = 0; tx < S.ntx; ++tx)
+        for (int ty = b0; ty < std::min(S.nty, b0 + band); ++ty) {
         const int x0 = tx * TX, y0 = ty * TY;
         const bool slab = touches_slab(0, x0, x0 + TX) || touches_slab(1, y0, y0 + TY);
         items.push_back({(zb[c + 1] - zb[c] + 4) * (slab ? 1.5 : 1.0), make_int4(x0, y0, zb[c], zb[c + 1])});
