@@ -192,6 +192,21 @@ int64_t fdtd_launch_count(const fdtd_ctx* ctx);
 /* Total grid extents. */
 int fdtd_dims(const fdtd_ctx* ctx, int32_t out[3]);
 
+/* max |f| over a contiguous DEVICE array of n fp32 values, written to *out_dev (DEVICE), for callers that cannot allocate:
+ * code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  Needs no context and no workspace,
+ * and calls no cudaMalloc / cudaFree or allocating library routine: the reduction's scratch (one partial maximum per thread
+ * block and a ticket counter) lives in a static device array of FDTD_NOALLOC_SCRATCH_BYTES that every GPU loading the library
+ * holds until exit.  One block reduces 65,536 values, so n is limited to FDTD_NOALLOC_MAX_ELEMS (2^30 values = 4 GiB; a
+ * 1024^3 field); a larger n returns FDTD_EINVAL with the limit in fdtd_last_error() and launches nothing.  Same value as
+ * fdtd_field_absmax over the same data (NaNs are ignored by both); n = 0 gives 0.  Runs on the CURRENT device, asynchronous
+ * on `stream` (a cudaStream_t; the result is in *out_dev once the stream has reached it).  All calls on one device share
+ * the scratch array, which keeps the last call's contents: the ticket is cleared by every call, the partials are rewritten
+ * before they are read.  Calls that overlap on the GPU (different streams, or graphs replayed concurrently) race on it:
+ * serialise them. */
+#define FDTD_NOALLOC_MAX_ELEMS (1ull << 30)
+#define FDTD_NOALLOC_SCRATCH_BYTES 65792
+int fdtd_absmax_noalloc(const float* in_dev, uint64_t n, float* out_dev, void* stream);
+
 /* Releases the context (not the workspace).  Synchronises the stream first. */
 int fdtd_destroy(fdtd_ctx* ctx);
 

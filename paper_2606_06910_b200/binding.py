@@ -25,7 +25,7 @@ FDTD_OK, FDTD_EINVAL, FDTD_EWORKSPACE, FDTD_ECUDA, FDTD_EUNSUPPORTED = 0, -1, -2
 EXPORTS = [
     "fdtd_workspace_bytes", "fdtd_create", "fdtd_set_model", "fdtd_set_sources", "fdtd_step", "fdtd_step_profiled", "fdtd_get_field",
     "fdtd_get_field_box", "fdtd_set_field", "fdtd_get_field_f64", "fdtd_set_field_f64", "fdtd_get_psi_f64", "fdtd_fill_hash", "fdtd_get_psi", "fdtd_field_absmax", "fdtd_cpml_table",
-    "fdtd_coeffs", "fdtd_time_block_stats", "fdtd_kernel_in_use", "fdtd_launch_count", "fdtd_dims", "fdtd_destroy", "fdtd_last_error",
+    "fdtd_coeffs", "fdtd_absmax_noalloc", "fdtd_time_block_stats", "fdtd_kernel_in_use", "fdtd_launch_count", "fdtd_dims", "fdtd_destroy", "fdtd_last_error",
 ]
 
 
@@ -73,6 +73,7 @@ def _load():
     L.fdtd_create.argtypes = [C.POINTER(fdtd_params)]
     L.fdtd_set_model.argtypes = [vp, vp, vp]
     L.fdtd_set_sources.argtypes = [vp, i32, vp, vp, i32]
+    L.fdtd_absmax_noalloc.argtypes = [vp, u64, vp, vp]
     L.fdtd_step.argtypes = [vp, i32]
     L.fdtd_step_profiled.argtypes = [vp, i32, vp]
     L.fdtd_get_field.argtypes = [vp, i32, vp]
@@ -106,6 +107,16 @@ def last_error():
 def _check(rc, what):
     if rc != 0:
         raise FdtdError("%s failed (%d): %s" % (what, rc, last_error()))
+
+
+FDTD_NOALLOC_MAX_ELEMS = 1 << 30
+
+
+def fdtd_absmax_noalloc(in_dev_ptr, n, out_dev_ptr, stream_ptr=0):
+    """max |f| of n fp32 values at device address in_dev_ptr into the device float at out_dev_ptr, on the current device,
+    asynchronous on the stream; allocates nothing (static device scratch, n <= FDTD_NOALLOC_MAX_ELEMS)."""
+    _check(lib.fdtd_absmax_noalloc(C.c_void_p(int(in_dev_ptr)), C.c_uint64(int(n)), C.c_void_p(int(out_dev_ptr)), C.c_void_p(int(stream_ptr))),
+           "fdtd_absmax_noalloc")
 
 
 def fdtd_coeffs():

@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <thread>
 #include <algorithm>
@@ -1350,6 +1351,101 @@ int fdtd_cpml_table(fdtd_ctx* c, int32_t axis, int32_t half, float* a, float* b,
   const AxisTable& t = c->tabs[half ? 0 : 1][axis];
   const size_t n = (size_t)c->G.gn[axis];
   memcpy(a, t.a.data(), n * 4); memcpy(b, t.b.data(), n * 4); memcpy(ik, t.ik.data(), n * 4);
+  return FDTD_OK;
+}
+
+}  // extern "C"
+
+// ---- fdtd_absmax_noalloc: max |f| of a caller-owned device array with no allocation at all ---------------------------------
+// The variant of absmax_kernel for callers that cannot allocate (CUDA graph capture, serving loops): absmax_kernel reduces
+// into a scratch word of the context's workspace with atomicMax; this one keeps its scratch — one ticket counter and one
+// partial maximum per thread block — in a file-scope device array of fixed size that every GPU loading the library holds
+// until exit (FDTD_NOALLOC_SCRATCH_BYTES, 64.25 KB).  Block b reduces the fixed chunk [b, b+1) x NOALLOC_CHUNK of the
+// input into partial[b]; the last block to finish (ticket) reduces the partials, writes the result and re-arms the ticket.
+namespace {
+constexpr int NOALLOC_MAX_BLOCKS = 16384;                 // partial maxima held by the static scratch
+constexpr int NOALLOC_CHUNK = 65536;                      // floats per block: 256 threads x 64 float4
+constexpr int NOALLOC_HEAD = 64;                          // words before the partials: word 0 is the ticket counter
+static_assert((uint64_t)NOALLOC_MAX_BLOCKS * NOALLOC_CHUNK == FDTD_NOALLOC_MAX_ELEMS, "header and kernel disagree on the limit");
+static_assert((NOALLOC_HEAD + NOALLOC_MAX_BLOCKS) * 4 == FDTD_NOALLOC_SCRATCH_BYTES, "header and kernel disagree on the scratch size");
+// In host code this name is a host-side stand-in, not a device address: the host gets the address from cudaGetSymbolAddress.
+static __device__ __align__(256) unsigned int g_noalloc_scratch[NOALLOC_HEAD + NOALLOC_MAX_BLOCKS];
+
+__global__ void __launch_bounds__(256) absmax_noalloc_kernel(const float* __restrict__ in, unsigned long long n, unsigned int* scratch,
+                                                             float* __restrict__ out) {
+  __shared__ float s_m[8];
+  __shared__ bool s_last;
+  const unsigned long long lo = (unsigned long long)blockIdx.x * NOALLOC_CHUNK;
+  const unsigned long long hi = lo + NOALLOC_CHUNK < n ? lo + NOALLOC_CHUNK : n;
+  float m = 0.f;
+  if ((reinterpret_cast<uintptr_t>(in) & 15) == 0) {       // lo is a multiple of 4 floats: whole float4s, then a scalar tail
+    const unsigned long long v0 = lo >> 2, v1 = hi >> 2;
+    for (unsigned long long t = v0 + threadIdx.x; t < v1; t += 256) {
+      const float4 f = __ldg(reinterpret_cast<const float4*>(in) + t);
+      m = fmaxf(m, fmaxf(fmaxf(fabsf(f.x), fabsf(f.y)), fmaxf(fabsf(f.z), fabsf(f.w))));
+    }
+    for (unsigned long long t = (v1 << 2) + threadIdx.x; t < hi; t += 256) m = fmaxf(m, fabsf(__ldg(in + t)));
+  } else {
+    for (unsigned long long t = lo + threadIdx.x; t < hi; t += 256) m = fmaxf(m, fabsf(__ldg(in + t)));
+  }
+  for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0) s_m[threadIdx.x >> 5] = m;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < 8; ++w) m = fmaxf(m, s_m[w]);
+    scratch[NOALLOC_HEAD + blockIdx.x] = __float_as_uint(m);
+    __threadfence();                                       // the partial is visible before the ticket is taken
+    s_last = atomicAdd(&scratch[0], 1u) == gridDim.x - 1;
+  }
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  float r = 0.f;
+  for (unsigned int b = threadIdx.x; b < gridDim.x; b += 256) r = fmaxf(r, __uint_as_float(((volatile unsigned int*)scratch)[NOALLOC_HEAD + b]));
+  for (int o = 16; o > 0; o >>= 1) r = fmaxf(r, __shfl_xor_sync(0xffffffffu, r, o));
+  if ((threadIdx.x & 31) == 0) s_m[threadIdx.x >> 5] = r;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < 8; ++w) r = fmaxf(r, s_m[w]);
+    *out = r;
+    scratch[0] = 0u;                                       // re-armed for the next call on this device
+  }
+}
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+unsigned int* g_noalloc_ptr[NOALLOC_MAX_DEVICES] = {nullptr};   // device address of g_noalloc_scratch, per device ordinal
+std::mutex g_noalloc_mutex;
+}  // namespace
+
+extern "C" {
+
+int fdtd_absmax_noalloc(const float* in_dev, uint64_t n, float* out_dev, void* stream) {
+  if (!out_dev || (!in_dev && n > 0)) { set_err("fdtd_absmax_noalloc: null pointer"); return FDTD_EINVAL; }
+  if (n > (uint64_t)FDTD_NOALLOC_MAX_ELEMS) {
+    set_err("fdtd_absmax_noalloc: " + std::to_string((unsigned long long)n) + " elements exceed the maximum of " +
+            std::to_string((unsigned long long)FDTD_NOALLOC_MAX_ELEMS) + " that the static scratch array supports");
+    return FDTD_EINVAL;
+  }
+  int dev = -1;
+  CK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) { set_err("fdtd_absmax_noalloc: device ordinal out of range"); return FDTD_EINVAL; }
+  unsigned int* scratch = nullptr;
+  {
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_ptr[dev]) {                            // set-up, once per device, with that device current
+      void* ptr = nullptr;
+      CK(cudaGetSymbolAddress(&ptr, g_noalloc_scratch));
+      g_noalloc_ptr[dev] = (unsigned int*)ptr;
+    }
+    scratch = g_noalloc_ptr[dev];
+  }
+  cudaStream_t st = (cudaStream_t)stream;
+  // The ticket must start at zero.  The kernel re-arms it, but a call that died half-way would leave it armed wrongly, so it
+  // is cleared here as well (a memset node on the stream: no allocation).  The partials are overwritten before they are read.
+  CK(cudaMemsetAsync(scratch, 0, NOALLOC_HEAD * 4, st));
+  const unsigned int blocks = n == 0 ? 1u : (unsigned int)((n + NOALLOC_CHUNK - 1) / NOALLOC_CHUNK);
+  absmax_noalloc_kernel<<<blocks, 256, 0, st>>>(in_dev, (unsigned long long)n, scratch, out_dev);
+  CK(cudaGetLastError());
   return FDTD_OK;
 }
 
