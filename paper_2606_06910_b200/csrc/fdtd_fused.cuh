@@ -376,7 +376,8 @@ __device__ __forceinline__ void fused_plane(const DomainView& D, const OutSet& O
 // Planes [k, kend) of an item.  Both rings stay in canonical order (oldest entry at index 0): they are shifted by one entry
 // per plane (56 register moves).  Renaming instead of moving needs the body unrolled 8x (or 4x / 2x with a rotation per
 // group), and every unrolled form measured slower than this one (8x: 2.06 instead of 1.44 ms at 552^3, 4x: 1.51, 2x: 1.50):
-// the body must stay resident in the instruction cache, and the kernel is not bound by issue slots.
+// the body must stay resident in the instruction cache, and the kernel is not bound by issue slots.  Re-measured on the final
+// build of round 2: the 2x form has 8.6 % fewer instructions per plane and is 6 % slower at 1600^3 (profiles/r02_ncu_step_fused.md).
 template <bool ZS, int XS, int YS, int V>
 __device__ __forceinline__ void fused_run(const DomainView& D, const OutSet& O, const float* smem, float* ebuf, const FusedBars& Q,
                                           const TabCache& T, const MainK& K, MainState<XS, YS>& C, int k, int kend) {
